@@ -1,0 +1,173 @@
+/*
+ * mred.h -- C ABI of the B200 (sm_100a) image-reduction hot path of arXiv 2008.11486
+ *           ("GPU-accelerated Image Reduction Pipeline", PAPER.md).
+ *
+ * The calls follow the paper's problem statement: overscan cutout, bias subtraction, dark
+ * subtraction, flat fielding, alignment by bicubic-spline sub-pixel shift and sigma-clipped-mean
+ * co-adding, plus the two steps the north star adds around them (master
+ * frame construction, image-based offset estimation).  The paper prints no formulas; the exact
+ * definition of every result is DESIGN.md section 3 (readings O1-O6, Q1-Q24).
+ *
+ * Conventions (all calls):
+ *  - Every array pointer is DEVICE memory owned by the caller unless the comment says "host".
+ *    The library never allocates, frees or retains a pointer and keeps no global mutable state
+ *    (apart from the last CUDA error code, see mred_last_cuda_error); calls on different
+ *    streams are independent.
+ *  - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *    stream) and the call returns WITHOUT synchronising, except mred_reduce_host which
+ *    returns after its device->host copies are enqueued (also not synchronised).
+ *  - Device array pointers must be 16-byte aligned (MRED_EALIGN otherwise).
+ *  - Layout: raw frames uint16 [n][H][W], x fastest; image planes [h][w], x fastest; stacks
+ *    [n][h][w].  Origin lower-left, X horizontal, Y vertical; row y=0 is first
+ *    in memory.
+ *  - Return value: MRED_OK (0) or a negative mred_status; never throws, never aborts.  On error
+ *    nothing has been enqueued unless the status is MRED_ECUDA.
+ *  - `ws` is caller-owned device scratch of at least mred_workspace_bytes(call, geom, n) bytes,
+ *    16-byte aligned; its contents are undefined afterwards and it must not be shared by calls
+ *    that may run concurrently.
+ *  - Frame counts: 1 <= n <= MRED_MAX_STACK (255) for every per-pixel-column call.
+ */
+#ifndef MRED_H
+#define MRED_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MRED_MAX_STACK 255
+#define MRED_MAX_LAG 256
+
+typedef struct {
+    int32_t W, H;         /* raw frame size, x fastest (1074 x 1024 incl. overscan)   */
+    int32_t os_x0, os_x1; /* overscan columns [os_x0, os_x1) over all H rows; equal -> level = 0     */
+    int32_t x0, y0, w, h; /* image rectangle kept by the overscan cutout               */
+} mred_geom;
+
+typedef enum { MRED_MEDIAN = 0, MRED_MEAN = 1, MRED_SIGCLIP = 2 } mred_combine;
+
+typedef struct {
+    int32_t mode;     /* mred_combine                                                             */
+    float ksigma;     /* clip threshold in sigma (SIGCLIP only), e.g. 3.0                          */
+    int32_t max_iter; /* maximum number of clip passes (SIGCLIP only), e.g. 3; 0 = plain mean      */
+} mred_comb_opts;
+
+typedef enum {
+    MRED_OK = 0,
+    MRED_EINVAL = -1,     /* null pointer, bad shape/geometry/count/option                          */
+    MRED_EALIGN = -2,     /* a device pointer is not 16-byte aligned                                */
+    MRED_EWORKSPACE = -3, /* ws is null or smaller than mred_workspace_bytes()                      */
+    MRED_ECUDA = -4       /* a CUDA runtime call failed; see mred_last_cuda_error()                 */
+} mred_status;
+
+typedef enum {
+    MRED_CALL_BUILD_MASTERS = 0,
+    MRED_CALL_CALIBRATE = 1,
+    MRED_CALL_ESTIMATE_SHIFTS = 2,
+    MRED_CALL_RESAMPLE = 3,
+    MRED_CALL_COADD = 4,
+    MRED_CALL_REDUCE = 5
+} mred_call;
+
+/*
+ * Master bias / dark / flat (O2; the paper uses masters but does not describe their
+ * construction).  With L_k the overscan level of each input frame (O1: exact
+ * integer mean of its overscan pixels) and comb = per-pixel median / mean / sigma-clipped mean:
+ *     MB = comb_k(B_k - L_k)
+ *     MD = comb_k(D_k - L_k - MB)                                   [ADU at t_dark]
+ *     G_k = F_k - L_k - MB - (t_flat/t_dark) MD ,  MF = comb_k(G_k/<G_k>) / <comb_k(..)>,  <MF> = 1
+ * bias/dark/flat: uint16 [nb|nd|nf][H][W].  MB, MD, MF: float32 [h][w] outputs.
+ */
+int mred_build_masters(const mred_geom *geom, const uint16_t *bias, int nb, const uint16_t *dark, int nd,
+                       float t_dark, const uint16_t *flat, int nf, float t_flat, const mred_comb_opts *opts,
+                       float *MB, float *MD, float *MF, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * Overscan cutout + level subtraction + bias/dark subtraction + flat fielding in one pass over
+ * the uint16 input (O1, O3):
+ *     out_k = (raw_k - L_k - MB - dark_scale * MD) / MF   on the image rectangle;  MF <= 0 or
+ *     non-finite -> 0.   dark_scale = t_sci / t_dark.
+ * raw: uint16 [n][H][W]; out: float32 [n][h][w]; level_out: float64 [n] (device, nullable)
+ * receives L_k.  n >= 1 (no upper bound other than memory).
+ */
+int mred_calibrate(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
+                   const float *MD, const float *MF, float *out, double *level_out, void *ws, size_t ws_bytes,
+                   void *stream);
+
+/*
+ * Per-frame offset relative to frame `ref_index` from marginal profiles (O4; replaces
+ * the WCS-header path of PAPER.md L69/L99): mean row/column profiles over pixels with
+ * badmask == 0, median-subtracted, 1-D cross-correlation over lags -max_lag..max_lag, integer
+ * argmax + 3-point parabola.  (dx, dy) is the displacement of frame k's CONTENT relative to the
+ * reference: a source at (x, y) in the reference sits at (x+dx, y+dy) in frame k.
+ * frames: float32 [n][h][w]; badmask: uint8 [h][w], nullable; ishift: int32 [n][2] (ix, iy);
+ * shift: float64 [n][2] (dx, dy); both device.  0 <= max_lag <= MRED_MAX_LAG, max_lag < min(w,h).
+ */
+int mred_estimate_shifts(const float *frames, int n, int w, int h, int ref_index, int max_lag,
+                         const uint8_t *badmask, int32_t *ishift, double *shift, void *ws, size_t ws_bytes,
+                         void *stream);
+
+/*
+ * Sub-pixel shift by bicubic (tensor-product natural cubic) spline interpolation (PAPER.md L63,
+ * L107, L164, L266; O5):  out_k(x, y) = spline_k(x - sx[k], y - sy[k]); pixels whose
+ * source lies outside the frame get `fill`.  An axis whose shift has zero fractional part is a
+ * pure integer translation, so (0, 0) is the bit-exact identity.  To align frame k onto the
+ * reference use (sx, sy) = (-dx, -dy) of mred_estimate_shifts.
+ * in/out: float32 [n][h][w] (must not overlap); sx, sy: HOST float64 [n];
+ * footprint: HOST int32 [n][4] output {x_lo, x_hi, y_lo, y_hi} inclusive (nullable) --
+ * written before the call returns.  w, h >= 4.
+ */
+int mred_resample(const float *in, int n, int w, int h, const double *sx, const double *sy, float fill,
+                  float *out, int32_t *footprint, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * Per-pixel combine along the stack axis (O6) over the
+ * frames whose footprint contains the pixel: median, mean, or ksigma-clipped mean (mean-centred,
+ * population sigma, keep |v-mu| <= k sigma, <= max_iter passes, early stop).
+ * stack: float32 [n][h][w]; footprint: HOST int32 [n][4] (nullable = every frame covers every
+ * pixel); out: float32 [h][w]; count: uint16 [h][w] number of frames used (nullable);
+ * rejmask: uint32 [ceil(n/32)][h][w], bit k%32 of word k/32 set iff frame k was NOT used
+ * (nullable).  No covering frame -> value 0, count 0.
+ */
+int mred_coadd(const float *stack, int n, int w, int h, const int32_t *footprint, const mred_comb_opts *opts,
+               float *out, uint16_t *count, uint32_t *rejmask, void *stream);
+
+/*
+ * The whole science path for one group, device-resident and chained without host round trips:
+ * calibrate -> estimate_shifts (vs ref_index) -> resample by (-dx, -dy) -> coadd.
+ * raw: uint16 [n][H][W].  shift_out: float64 [n][2] device (nullable) receives (dx, dy);
+ * footprint_out: int32 [n][4] device (nullable).  Other arguments as in the single calls.
+ */
+int mred_reduce(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
+                const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
+                float fill, const mred_comb_opts *opts, float *out, uint16_t *count, uint32_t *rejmask,
+                double *shift_out, int32_t *footprint_out, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * Same as mred_reduce with HOST input and output buffers: raw_host (uint16 [n][H][W], ideally
+ * pinned) is copied to the device inside the call, out_host (float32 [h][w]), count_host
+ * (uint16 [h][w], nullable) and shift_host (float64 [n][2], nullable) are copied back; all on
+ * `stream`, nothing synchronised.  Masters and badmask stay device pointers.  ws needs
+ * mred_workspace_bytes(MRED_CALL_REDUCE, geom, n) + the staging the call adds itself, i.e. use
+ * mred_reduce_host_workspace_bytes().
+ */
+int mred_reduce_host(const mred_geom *geom, const uint16_t *raw_host, int n, float dark_scale, const float *MB,
+                     const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
+                     float fill, const mred_comb_opts *opts, float *out_host, uint16_t *count_host,
+                     double *shift_host, void *ws, size_t ws_bytes, void *stream);
+
+/* Scratch size for one call (call = mred_call).  geom may be NULL for the calls that take w, h
+ * directly, in which case pass them through a mred_geom with only w, h set. */
+size_t mred_workspace_bytes(int call, const mred_geom *geom, int n);
+size_t mred_reduce_host_workspace_bytes(const mred_geom *geom, int n);
+
+const char *mred_strerror(int status);
+int mred_last_cuda_error(void); /* cudaError_t of the most recent failing runtime call, else 0 */
+const char *mred_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MRED_H */
