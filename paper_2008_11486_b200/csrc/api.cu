@@ -1,0 +1,242 @@
+// api.cu -- the extern "C" boundary declared in include/mred.h: argument validation, workspace
+// carving and kernel launches.  No allocation, no synchronisation, no global state except the last
+// CUDA error code.
+#include "common.cuh"
+#include <atomic>
+#include <math.h>
+
+namespace mred {
+
+static std::atomic<int> g_last_cuda_error{0};
+void set_cuda_error(cudaError_t e) { g_last_cuda_error.store((int)e); }
+
+static bool opts_ok(const mred_comb_opts* o)
+{
+    if (!o) return false;
+    if (o->mode != MRED_MEDIAN && o->mode != MRED_MEAN && o->mode != MRED_SIGCLIP) return false;
+    if (o->mode == MRED_SIGCLIP && (!(o->ksigma >= 0.f) || o->max_iter < 0)) return false;
+    return true;
+}
+
+struct ReduceWs {
+    float* cal;               // [n][h][w]
+    float* reg;               // [n][h][w]
+    unsigned long long* os;   // [n]
+    int32_t* ishift;          // [n][2]
+    double* shift;            // [n][2]
+    int32_t* fp;              // [n][4]
+    void* est;                // estimate workspace
+    size_t bytes;
+};
+
+static ReduceWs carve_reduce(void* ws, const Geom& g, int n)
+{
+    ReduceWs r;
+    char* p = static_cast<char*>(ws);
+    auto take = [&](size_t b) { char* q = p; p += align_up(b, 256); return q; };
+    const size_t np = (size_t)g.w * g.h;
+    r.cal = reinterpret_cast<float*>(take(4 * np * n));
+    r.reg = reinterpret_cast<float*>(take(4 * np * n));
+    r.os = reinterpret_cast<unsigned long long*>(take(8 * (size_t)n));
+    r.ishift = reinterpret_cast<int32_t*>(take(8 * (size_t)n));
+    r.shift = reinterpret_cast<double*>(take(16 * (size_t)n));
+    r.fp = reinterpret_cast<int32_t*>(take(16 * (size_t)n));
+    r.est = take(estimate_ws_bytes(g.w, g.h, n));
+    r.bytes = (size_t)(p - static_cast<char*>(ws));
+    return r;
+}
+
+struct HostWs {
+    uint16_t* raw;   // [n][H][W]
+    float* out;      // [h][w]
+    uint16_t* count; // [h][w]
+    void* reduce;
+    size_t bytes;
+};
+
+static HostWs carve_host(void* ws, const Geom& g, int n)
+{
+    HostWs r;
+    char* p = static_cast<char*>(ws);
+    auto take = [&](size_t b) { char* q = p; p += align_up(b, 256); return q; };
+    const size_t np = (size_t)g.w * g.h;
+    r.raw = reinterpret_cast<uint16_t*>(take(2 * (size_t)g.W * g.H * n));
+    r.out = reinterpret_cast<float*>(take(4 * np));
+    r.count = reinterpret_cast<uint16_t*>(take(2 * np));
+    r.reduce = take(carve_reduce(nullptr, g, n).bytes);
+    r.bytes = (size_t)(p - static_cast<char*>(ws));
+    return r;
+}
+
+}  // namespace mred
+
+using namespace mred;
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+const char* mred_version(void) { return "mred 0.1 (sm_100a)"; }
+
+int mred_last_cuda_error(void) { return g_last_cuda_error.load(); }
+
+const char* mred_strerror(int status)
+{
+    switch (status) {
+        case MRED_OK: return "ok";
+        case MRED_EINVAL: return "invalid argument (null pointer, shape, geometry, count or option)";
+        case MRED_EALIGN: return "device pointer not 16-byte aligned";
+        case MRED_EWORKSPACE: return "workspace missing or too small";
+        case MRED_ECUDA: return "CUDA runtime error (see mred_last_cuda_error)";
+        default: return "unknown status";
+    }
+}
+
+size_t mred_workspace_bytes(int call, const mred_geom* geom, int n)
+{
+    if (!geom || n < 1) return 0;
+    const Geom g = to_geom(geom);
+    switch (call) {
+        case MRED_CALL_BUILD_MASTERS: return masters_ws_bytes(g, n);
+        case MRED_CALL_CALIBRATE: return align_up(8 * (size_t)n, 16);
+        case MRED_CALL_ESTIMATE_SHIFTS: return estimate_ws_bytes(g.w, g.h, n);
+        case MRED_CALL_RESAMPLE: return 0;
+        case MRED_CALL_COADD: return 0;
+        case MRED_CALL_REDUCE: return carve_reduce(nullptr, g, n).bytes;
+        default: return 0;
+    }
+}
+
+size_t mred_reduce_host_workspace_bytes(const mred_geom* geom, int n)
+{
+    if (!geom || n < 1) return 0;
+    return carve_host(nullptr, to_geom(geom), n).bytes;
+}
+
+int mred_build_masters(const mred_geom* geom, const uint16_t* bias, int nb, const uint16_t* dark, int nd,
+                       float t_dark, const uint16_t* flat, int nf, float t_flat, const mred_comb_opts* opts,
+                       float* MB, float* MD, float* MF, void* ws, size_t ws_bytes, void* stream)
+{
+    if (!geom_ok(geom) || !bias || !dark || !flat || !MB || !MD || !MF || !opts_ok(opts)) return MRED_EINVAL;
+    if (nb < 1 || nd < 1 || nf < 1 || nb > MRED_MAX_STACK || nd > MRED_MAX_STACK || nf > MRED_MAX_STACK) return MRED_EINVAL;
+    if (!(t_dark > 0.f) || !(t_flat >= 0.f)) return MRED_EINVAL;
+    if (!aligned16(bias) || !aligned16(dark) || !aligned16(flat) || !aligned16(MB) || !aligned16(MD) || !aligned16(MF))
+        return MRED_EALIGN;
+    const Geom g = to_geom(geom);
+    int nmax = nb > nd ? nb : nd;
+    nmax = nmax > nf ? nmax : nf;
+    if (!ws || !aligned16(ws) || ws_bytes < masters_ws_bytes(g, nmax)) return MRED_EWORKSPACE;
+    return launch_build_masters(g, bias, nb, dark, nd, t_dark, flat, nf, t_flat, *opts, MB, MD, MF, ws,
+                                static_cast<cudaStream_t>(stream));
+}
+
+int mred_calibrate(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+                   const float* MD, const float* MF, float* out, double* level_out, void* ws, size_t ws_bytes,
+                   void* stream)
+{
+    if (!geom_ok(geom) || !raw || !MB || !MD || !MF || !out || n < 1 || n > 65535 * 8) return MRED_EINVAL;
+    if (!aligned16(raw) || !aligned16(MB) || !aligned16(MD) || !aligned16(MF) || !aligned16(out)) return MRED_EALIGN;
+    if (!ws || !aligned16(ws) || ws_bytes < 8 * (size_t)n) return MRED_EWORKSPACE;
+    const Geom g = to_geom(geom);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned long long* os = static_cast<unsigned long long*>(ws);
+    int rc = launch_frame_sums(raw, g, n, os, nullptr, st);
+    if (rc) return rc;
+    return launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, out, level_out, os, nullptr, st);
+}
+
+int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index, int max_lag,
+                         const uint8_t* badmask, int32_t* ishift, double* shift, void* ws, size_t ws_bytes,
+                         void* stream)
+{
+    if (!frames || !ishift || !shift || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1) return MRED_EINVAL;
+    if (w > 4096 || h > 4096) return MRED_EINVAL;   // profile length held in shared memory
+    if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= w || max_lag >= h)
+        return MRED_EINVAL;
+    if (!aligned16(frames) || !aligned16(ishift) || !aligned16(shift) || (badmask && !aligned16(badmask)))
+        return MRED_EALIGN;
+    if (!ws || !aligned16(ws) || ws_bytes < estimate_ws_bytes(w, h, n)) return MRED_EWORKSPACE;
+    return launch_estimate(frames, n, w, h, ref_index, max_lag, badmask, ishift, shift, ws,
+                           static_cast<cudaStream_t>(stream));
+}
+
+int mred_resample(const float* in, int n, int w, int h, const double* sx, const double* sy, float fill,
+                  float* out, int32_t* footprint, void* ws, size_t ws_bytes, void* stream)
+{
+    (void)ws; (void)ws_bytes;
+    if (!in || !out || !sx || !sy || n < 1 || n > MRED_MAX_STACK || w < 4 || h < 4 || in == out) return MRED_EINVAL;
+    for (int k = 0; k < n; ++k)
+        if (!isfinite(sx[k]) || !isfinite(sy[k]) || fabs(sx[k]) > 1.0e6 || fabs(sy[k]) > 1.0e6) return MRED_EINVAL;
+    if (!aligned16(in) || !aligned16(out)) return MRED_EALIGN;
+    if (footprint)
+        for (int k = 0; k < n; ++k) {
+            int lo, hi;
+            axis_footprint(w, sx[k], lo, hi);
+            footprint[4 * k] = lo; footprint[4 * k + 1] = hi;
+            axis_footprint(h, sy[k], lo, hi);
+            footprint[4 * k + 2] = lo; footprint[4 * k + 3] = hi;
+        }
+    return launch_resample(in, n, w, h, sx, sy, nullptr, fill, out, nullptr, static_cast<cudaStream_t>(stream));
+}
+
+int mred_coadd(const float* stack, int n, int w, int h, const int32_t* footprint, const mred_comb_opts* opts,
+               float* out, uint16_t* count, uint32_t* rejmask, void* stream)
+{
+    if (!stack || !out || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1 || !opts_ok(opts)) return MRED_EINVAL;
+    if (!aligned16(stack) || !aligned16(out) || (count && !aligned16(count)) || (rejmask && !aligned16(rejmask)))
+        return MRED_EALIGN;
+    return launch_coadd(stack, n, w, h, footprint, nullptr, *opts, out, count, rejmask,
+                        static_cast<cudaStream_t>(stream));
+}
+
+int mred_reduce(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+                const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
+                int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream)
+{
+    if (!geom_ok(geom) || !raw || !MB || !MD || !MF || !out || !opts_ok(opts)) return MRED_EINVAL;
+    if (n < 1 || n > MRED_MAX_STACK || geom->w < 4 || geom->h < 4 || geom->w > 4096 || geom->h > 4096) return MRED_EINVAL;
+    if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= geom->w || max_lag >= geom->h)
+        return MRED_EINVAL;
+    if (!aligned16(raw) || !aligned16(MB) || !aligned16(MD) || !aligned16(MF) || !aligned16(out) ||
+        (count && !aligned16(count)) || (rejmask && !aligned16(rejmask)) || (badmask && !aligned16(badmask)) ||
+        (shift_out && !aligned16(shift_out)) || (footprint_out && !aligned16(footprint_out)))
+        return MRED_EALIGN;
+    const Geom g = to_geom(geom);
+    if (!ws || !aligned16(ws) || ws_bytes < carve_reduce(nullptr, g, n).bytes) return MRED_EWORKSPACE;
+    const ReduceWs r = carve_reduce(ws, g, n);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc;
+    if ((rc = launch_frame_sums(raw, g, n, r.os, nullptr, st))) return rc;
+    if ((rc = launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, r.cal, nullptr, r.os, nullptr, st))) return rc;
+    double* shift = shift_out ? shift_out : r.shift;
+    int32_t* fp = footprint_out ? footprint_out : r.fp;
+    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, st))) return rc;
+    if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, st))) return rc;
+    return launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st);
+}
+
+int mred_reduce_host(const mred_geom* geom, const uint16_t* raw_host, int n, float dark_scale, const float* MB,
+                     const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                     const mred_comb_opts* opts, float* out_host, uint16_t* count_host, double* shift_host, void* ws,
+                     size_t ws_bytes, void* stream)
+{
+    if (!geom_ok(geom) || !raw_host || !out_host || n < 1 || n > MRED_MAX_STACK) return MRED_EINVAL;
+    const Geom g = to_geom(geom);
+    if (!ws || !aligned16(ws) || ws_bytes < carve_host(nullptr, g, n).bytes) return MRED_EWORKSPACE;
+    const HostWs hw = carve_host(ws, g, n);
+    const ReduceWs r = carve_reduce(hw.reduce, g, n);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t np = (size_t)g.w * g.h;
+    MRED_CUDA_TRY(cudaMemcpyAsync(hw.raw, raw_host, 2 * (size_t)g.W * g.H * n, cudaMemcpyHostToDevice, st));
+    int rc = mred_reduce(geom, hw.raw, n, dark_scale, MB, MD, MF, ref_index, max_lag, badmask, fill, opts, hw.out,
+                         count_host ? hw.count : nullptr, nullptr, r.shift, nullptr, hw.reduce,
+                         carve_reduce(nullptr, g, n).bytes, stream);
+    if (rc) return rc;
+    MRED_CUDA_TRY(cudaMemcpyAsync(out_host, hw.out, 4 * np, cudaMemcpyDeviceToHost, st));
+    if (count_host) MRED_CUDA_TRY(cudaMemcpyAsync(count_host, hw.count, 2 * np, cudaMemcpyDeviceToHost, st));
+    if (shift_host) MRED_CUDA_TRY(cudaMemcpyAsync(shift_host, r.shift, 16 * (size_t)n, cudaMemcpyDeviceToHost, st));
+    return MRED_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"
