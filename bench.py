@@ -1,0 +1,369 @@
+"""bench.py -- reduced science frames/s of the whole hot path (build_masters + calibrate + estimate_shifts +
+resample + coadd) on seeded synthetic MITSuME-like frames, one process per GPU.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for what each key means.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+METRIC = "reduced frames/s (1074x1024 u16 calib+align+coadd)"
+UNIT = "frames/s"
+MAX_LAG = {1: 16, 2: 32, 3: 40, 4: 16, 5: 64}
+STAGES = ["calibrate", "estimate_shifts", "resample", "coadd"]
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default: configs[1])")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg):
+    sp = synth.CONFIGS[cfg]
+    g = sp["geom"]
+    return "config %d: %d group(s) x (%d science + %d/%d/%d bias/dark/flat) of %dx%d u16" % (
+        cfg, sp["groups"], sp["n_sci"], sp["n_master"], sp["n_master"], sp["n_master"], g.W, g.H)
+
+
+def make_groups(cfg, rank):
+    """All groups of the config for this rank (weak scaling: every rank gets its own full copy, seeded apart)."""
+    sp = synth.CONFIGS[cfg]
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(8, sp["groups"])) as ex:
+        return list(ex.map(lambda gi: synth.make_group(cfg, gi + 100 * rank), range(sp["groups"])))
+
+
+def stage_bytes(g, n, nm, want_mask_words=0):
+    """Algorithmic bytes per call (every input byte read once, every output byte written once); DESIGN.md."""
+    raw, img = 2 * g.W * g.H, 4 * g.w * g.h
+    return {
+        "build_masters": 3 * nm * raw + 3 * img,
+        "calibrate": n * (raw + img) + 3 * img,
+        "estimate_shifts": n * img,
+        "resample": 2 * n * img,
+        "coadd": n * img + img + img // 2 + want_mask_words * img,
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) >= 9:
+                for nm, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ------------------------------------------------------------------------------------------------
+def time_oracle_group(grp, max_lag, n_sci=None):
+    """One group through the oracle as it stands, single thread.  Returns (seconds, frames, per-stage s)."""
+    import oracle
+    oracle.lib()
+    g = grp.geom
+    sci = grp.sci if n_sci is None else grp.sci[:n_sci]
+    t = {}
+    t0 = time.perf_counter()
+    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
+    t["build_masters"] = time.perf_counter() - t0
+    t1 = time.perf_counter()
+    c = oracle.calibrate(g, sci, grp.t_sci / grp.t_dark, m.MB, m.MD, m.MF)
+    t["calibrate"] = time.perf_counter() - t1
+    t1 = time.perf_counter()
+    e = oracle.estimate_shifts(c.out, 0, max_lag, badmask=grp.badmask)
+    t["estimate_shifts"] = time.perf_counter() - t1
+    t1 = time.perf_counter()
+    r = oracle.resample(c.out, -e.shift[:, 0], -e.shift[:, 1])
+    t["resample"] = time.perf_counter() - t1
+    t1 = time.perf_counter()
+    oracle.coadd(r.out, r.footprint, mode=grp.coadd)
+    t["coadd"] = time.perf_counter() - t1
+    return time.perf_counter() - t0, sci.shape[0], t
+
+
+def oracle_sample_plan(cfg):
+    """Bounded sample of the workload for the CPU leg: one group, frame counts cut so it takes ~10-30 s."""
+    sp = synth.CONFIGS[cfg]
+    if sp["geom"].w > 2048:
+        return dict(n_sci=2, n_master=2)           # 4128 x 4096 frames: ~2.7 s per science frame
+    return dict(n_sci=min(sp["n_sci"], 20), n_master=min(sp["n_master"], 10))
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config/metric, each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.config
+    plan = oracle_sample_plan(cfg)
+    grp = synth.make_group(cfg, 0, **plan)
+    steps = max(1, min(args.steps, 3))
+    warm = 1 if args.warmup > 0 else 0
+    for _ in range(warm):
+        time_oracle_group(grp, MAX_LAG[cfg], n_sci=2)
+    tot, frames = 0.0, 0
+    for _ in range(steps):
+        s, n, _ = time_oracle_group(grp, MAX_LAG[cfg])
+        tot += s
+        frames += n
+    val = frames / tot
+    sample = "1 group, %d science + %d/%d/%d masters per step (config %d shapes)" % (
+        plan["n_sci"], plan["n_master"], plan["n_master"], plan["n_master"], cfg)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "ms_per_step": 1e3 * tot / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+KERNELS_PER_BUILD_MASTERS = 8    # 3 x k_frame_sums, k_masters_bd, k_flat_means, k_masters_f, k_mf_mean, k_mf_scale
+KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2008_11486_b200 import binding as mred
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    devs = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=devs)
+    mred.lib()
+    cfg = args.config
+    sp = synth.CONFIGS[cfg]
+    g = sp["geom"]
+    n, nm, G = sp["n_sci"], sp["n_master"], sp["groups"]
+    groups = make_groups(cfg, rank)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    host = [dict(bias=pin(gr.bias), dark=pin(gr.dark), flat=pin(gr.flat), sci=pin(gr.sci)) for gr in groups]
+    devg = [{k: v.to(devs) for k, v in h.items()} for h in host]
+    bad = [torch.from_numpy(gr.badmask).to(devs) if gr.badmask is not None else None for gr in groups]
+    words = (n + 31) // 32 if sp["stress"] else 0
+    plans = [mred.ReducePlan(g, n, device=devs, want_mask=bool(words)) for _ in range(G)]
+    mws = torch.empty(mred.workspace_bytes(mred.CALL_BUILD_MASTERS, g, nm), dtype=torch.uint8, device=devs)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=devs)   # > 2 x L2 (126 MB)
+    mode = groups[0].coadd
+    lag = MAX_LAG[cfg]
+    scale = groups[0].t_sci / groups[0].t_dark
+    nstage = len(STAGES)
+
+    def step(ev_m, ev_s):
+        """One pass of the whole hot path over the batch: every group, masters then the chained science path."""
+        for gi in range(G):
+            d = devg[gi]
+            if ev_m is not None:
+                ev_m[gi][0].record()
+            MB, MD, MF = mred.build_masters(g, d["bias"], d["dark"], groups[gi].t_dark, d["flat"], groups[gi].t_flat,
+                                            mode=mred.MEDIAN, ws=mws)
+            if ev_m is not None:
+                ev_m[gi][1].record()
+            mred.reduce(plans[gi], d["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode,
+                        events=None if ev_s is None else ev_s[gi])
+
+    def new_events():
+        E = lambda: torch.cuda.Event(enable_timing=True)
+        return [[E(), E()] for _ in range(G)], [[E() for _ in range(5)] for _ in range(G)]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.fill_(1)
+        step(None, None)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    wall0 = time.perf_counter()
+    step_ev, stage_ev = [], []
+    for _ in range(args.steps):
+        flush.fill_(1)                       # cold L2 before every timed step (not inside the step's events)
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        evm, evs = new_events()
+        s0.record()
+        step(evm, evs)
+        s1.record()
+        step_ev.append((s0, s1))
+        stage_ev.append((evm, evs))
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in step_ev]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=devs)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    frames_per_step = G * n * world
+    value = frames_per_step * args.steps / (total_ms * 1e-3)
+
+    # per-stage device times inside the timed region (average per call = per group)
+    sb = stage_bytes(g, n, nm, words)
+    st_ms = {k: [] for k in ["build_masters"] + STAGES}
+    for evm, evs in stage_ev:
+        for gi in range(G):
+            st_ms["build_masters"].append(evm[gi][0].elapsed_time(evm[gi][1]))
+            for i, nmst in enumerate(STAGES):
+                st_ms[nmst].append(evs[gi][i].elapsed_time(evs[gi][i + 1]))
+    peaks = {}
+    pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk_path):
+        peaks = json.load(open(pk_path))
+    peak, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json)") if "hbm_gbs" in peaks else (6650.0, "fallback")
+    stages = {}
+    for k, v in st_ms.items():
+        ms = float(np.mean(v))
+        gbs = sb[k] / (ms * 1e-3) / 1e9
+        stages[k] = {"ms_per_call": round(ms, 5), "algorithmic_MB": round(sb[k] / 1e6, 3), "GBps": round(gbs, 1),
+                     "frac": round(gbs / peak, 4)}
+    dom = max(STAGES, key=lambda k: np.sum(st_ms[k]))
+    kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_finalize, k_correlate)",
+            "resample": "k_resample", "coadd": "k_coadd"}[dom]
+    roof = {"bound": "hbm", "kernel": kern, "stage": dom, "achieved": stages[dom]["GBps"], "peak": peak,
+            "peak_source": peak_src, "unit": "GB/s", "frac": stages[dom]["frac"], "traffic": None,
+            "algorithmic_bytes_per_launch": sb[dom], "launch_ms": stages[dom]["ms_per_call"]}
+    sci_bytes = sum(sb[k] for k in STAGES)
+    sci_ms = sum(stages[k]["ms_per_call"] for k in STAGES)
+    e2e_roof = {"science_path_GBps": round(sci_bytes / (sci_ms * 1e-3) / 1e9, 1),
+                "science_path_frac": round(sci_bytes / (sci_ms * 1e-3) / 1e9 / peak, 4),
+                "whole_step_GBps": round((sci_bytes + sb["build_masters"]) * G / (total_ms / args.steps * 1e-3) / 1e9, 1)}
+
+    # end to end through the C ABI with HOST buffers (H2D of every input and D2H of the result inside the region)
+    e2e = None
+    if not args.no_e2e:
+        hplans = [mred.ReducePlan(g, n, device=devs, host=True) for _ in range(G)]
+        stg = [{k: torch.empty_like(v) for k, v in d.items() if k != "sci"} for d in devg]
+
+        def step_host():
+            for gi in range(G):
+                for k in ("bias", "dark", "flat"):
+                    stg[gi][k].copy_(host[gi][k], non_blocking=True)
+                MB, MD, MF = mred.build_masters(g, stg[gi]["bias"], stg[gi]["dark"], groups[gi].t_dark,
+                                                stg[gi]["flat"], groups[gi].t_flat, mode=mred.MEDIAN, ws=mws)
+                mred.reduce_host(hplans[gi], host[gi]["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode)
+        for _ in range(2):
+            step_host()
+        barrier()
+        ks = max(3, min(args.steps, 10))
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(ks):
+            step_host()
+        b.record()
+        barrier()
+        ems = a.elapsed_time(b)
+        if world > 1:
+            t = torch.tensor([ems], dtype=torch.float64, device=devs)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        raw = 2 * g.W * g.H
+        e2e = {"value": frames_per_step * ks / (ems * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": G * (n + 3 * nm) * raw,
+               "d2h_bytes_per_step": G * (4 * g.w * g.h + 2 * g.w * g.h + 16 * n), "steps": ks,
+               "api": "mred_build_masters + mred_reduce_host (pinned host uint16 in, host float32 co-add out)"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        plan = oracle_sample_plan(cfg)
+        grp = synth.make_group(cfg, 0, **plan)
+        s, nf, per = time_oracle_group(grp, lag)
+        cpu = {"value": nf / s, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "1 group, %d science + %d/%d/%d masters (config %d shapes), %.1f s" % (
+                   plan["n_sci"], plan["n_master"], plan["n_master"], plan["n_master"], cfg, s),
+               "stage_seconds": {k: round(v, 3) for k, v in per.items()}, "host_cores_available": os.cpu_count()}
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_name(cfg), "frames_per_step_per_gpu": G * n,
+                           "includes": "build_masters + calibrate + estimate_shifts + resample + coadd per group",
+                           "coadd": ["median", "mean", "sigclip 3.0 x3"][mode], "l2": "512 MB flush before every step",
+                           "parallelism": "groups sharded over ranks, no collective"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + KERNELS_PER_REDUCE),
+                "roofline": roof, "stages": stages, "path_roofline": e2e_roof, "cpu_baseline": cpu,
+                "wall_s_timed_region": round(wall, 4), "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU "
+                "stages on a TITAN X (Pascal) = ~870 frames/s (other hardware, other data; context only)"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

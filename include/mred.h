@@ -146,6 +146,17 @@ int mred_reduce(const mred_geom *geom, const uint16_t *raw, int n, float dark_sc
                 double *shift_out, int32_t *footprint_out, void *ws, size_t ws_bytes, void *stream);
 
 /*
+ * mred_reduce with stage markers: events is a HOST array of 5 cudaEvent_t (as void*, entries nullable)
+ * recorded on `stream` before calibrate and after calibrate, estimate_shifts, resample and coadd, so a
+ * caller can time each stage of the chained pass on the device.  events == NULL is mred_reduce.
+ */
+int mred_reduce_staged(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
+                       const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
+                       float fill, const mred_comb_opts *opts, float *out, uint16_t *count, uint32_t *rejmask,
+                       double *shift_out, int32_t *footprint_out, void *ws, size_t ws_bytes, void *stream,
+                       void *const *events);
+
+/*
  * Same as mred_reduce with HOST input and output buffers: raw_host (uint16 [n][H][W], ideally
  * pinned) is copied to the device inside the call, out_host (float32 [h][w]), count_host
  * (uint16 [h][w], nullable) and shift_host (float64 [n][2], nullable) are copied back; all on

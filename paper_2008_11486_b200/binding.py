@@ -19,7 +19,7 @@ CALL_BUILD_MASTERS, CALL_CALIBRATE, CALL_ESTIMATE_SHIFTS, CALL_RESAMPLE, CALL_CO
 MAX_STACK = 255
 
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
-           "mred_reduce", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
+           "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -218,16 +218,23 @@ class ReducePlan:
 
 
 def reduce(plan: ReducePlan, raw, dark_scale, MB, MD, MF, ref_index=0, max_lag=32, badmask=None, fill=0.0,
-           mode=SIGCLIP, ksigma=3.0, max_iter=3, stream=None):
-    """include/mred.h: mred_reduce (device-resident chained science path).  Results land in `plan`."""
+           mode=SIGCLIP, ksigma=3.0, max_iter=3, stream=None, events=None):
+    """include/mred.h: mred_reduce / mred_reduce_staged (device-resident chained science path).  Results land
+    in `plan`.  events: optional list of 5 torch.cuda.Event(enable_timing=True) recorded around the stages."""
     o = _opts(mode, ksigma, max_iter)
-    rc = lib().mred_reduce(C.byref(plan.g), _dev(raw, torch.uint16, "raw"), C.c_int(plan.n), C.c_float(dark_scale),
+    ev = C.c_void_p(None)
+    if events is not None:
+        for e in events:
+            if e.cuda_event == 0:      # torch creates the CUDA event lazily, on first record
+                e.record(torch.cuda.current_stream() if stream is None else stream)
+        ev = (C.c_void_p * 5)(*[C.c_void_p(e.cuda_event) for e in events])
+    rc = lib().mred_reduce_staged(C.byref(plan.g), _dev(raw, torch.uint16, "raw"), C.c_int(plan.n), C.c_float(dark_scale),
                            _dev(MB, torch.float32, "MB"), _dev(MD, torch.float32, "MD"), _dev(MF, torch.float32, "MF"),
                            C.c_int(ref_index), C.c_int(max_lag), _dev(badmask, torch.uint8, "badmask"),
                            C.c_float(fill), C.byref(o), _dev(plan.out, torch.float32, "out"),
                            _dev(plan.count, torch.uint16, "count"), _dev(plan.mask, torch.uint32, "rejmask"),
                            _dev(plan.shift, torch.float64, "shift"), _dev(plan.footprint, torch.int32, "footprint"),
-                           C.c_void_p(plan.ws.data_ptr()), C.c_size_t(plan.ws.numel()), _stream(stream))
+                           C.c_void_p(plan.ws.data_ptr()), C.c_size_t(plan.ws.numel()), _stream(stream), ev)
     _check(rc, "mred_reduce")
     return plan
 

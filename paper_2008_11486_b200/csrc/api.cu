@@ -188,10 +188,10 @@ int mred_coadd(const float* stack, int n, int w, int h, const int32_t* footprint
                         static_cast<cudaStream_t>(stream));
 }
 
-int mred_reduce(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
-                const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
-                const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
-                int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream)
+int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+                       const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                       const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
+                       int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream, void* const* events)
 {
     if (!geom_ok(geom) || !raw || !MB || !MD || !MF || !out || !opts_ok(opts)) return MRED_EINVAL;
     if (n < 1 || n > MRED_MAX_STACK || geom->w < 4 || geom->h < 4 || geom->w > 4096 || geom->h > 4096) return MRED_EINVAL;
@@ -206,13 +206,31 @@ int mred_reduce(const mred_geom* geom, const uint16_t* raw, int n, float dark_sc
     const ReduceWs r = carve_reduce(ws, g, n);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc;
+#define MRED_STAGE_EVENT(i) \
+    do { if (events && events[i]) MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[i]), st)); } while (0)
+    MRED_STAGE_EVENT(0);
     if ((rc = launch_frame_sums(raw, g, n, r.os, nullptr, st))) return rc;
     if ((rc = launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, r.cal, nullptr, r.os, nullptr, st))) return rc;
+    MRED_STAGE_EVENT(1);
     double* shift = shift_out ? shift_out : r.shift;
     int32_t* fp = footprint_out ? footprint_out : r.fp;
     if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, st))) return rc;
+    MRED_STAGE_EVENT(2);
     if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, st))) return rc;
-    return launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st);
+    MRED_STAGE_EVENT(3);
+    if ((rc = launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st))) return rc;
+    MRED_STAGE_EVENT(4);
+#undef MRED_STAGE_EVENT
+    return MRED_OK;
+}
+
+int mred_reduce(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+                const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
+                int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream)
+{
+    return mred_reduce_staged(geom, raw, n, dark_scale, MB, MD, MF, ref_index, max_lag, badmask, fill, opts, out, count,
+                              rejmask, shift_out, footprint_out, ws, ws_bytes, stream, nullptr);
 }
 
 int mred_reduce_host(const mred_geom* geom, const uint16_t* raw_host, int n, float dark_scale, const float* MB,
