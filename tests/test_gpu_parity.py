@@ -34,11 +34,20 @@ def host(t):
     return t.cpu().numpy()
 
 
-def assert_close(got, ref, what=""):
+def assert_close(got, ref, what="", local=0):
+    """|d| <= 1e-3 + 1e-5 |ref| (Q18).  local = r > 0 (resample only, Q18b): |ref| is replaced by its
+    maximum over the (2r+1)^2 neighbourhood in the same plane, because the spline prefilter is a linear
+    operator that mixes neighbours with weights 0.268^d: float32 rounding is relative to the largest neighbour
+    (a 65535-ADU saturated pixel next to 1000-ADU sky), not to the value that remains after cancellation."""
     got = np.asarray(got, np.float64)
     ref = np.asarray(ref, np.float64)
     d = np.abs(got - ref)
-    tol = 1e-3 + 1e-5 * np.abs(ref)
+    mag = np.abs(ref)
+    if local:
+        from scipy.ndimage import maximum_filter
+        size = [1] * (ref.ndim - 2) + [2 * local + 1, 2 * local + 1]
+        mag = maximum_filter(mag, size=size, mode="nearest")
+    tol = 1e-3 + 1e-5 * mag
     bad = d > tol
     assert not bad.any(), "%s: %d of %d outside tolerance, max |d| = %g, max ratio = %g" % (
         what, bad.sum(), bad.size, d.max(), (d / tol).max())
@@ -247,7 +256,7 @@ def test_resample_parity(shape):
     out, fp = mred.resample(dev(img), sx, sy, fill=-5.0)
     assert np.array_equal(fp, ref.footprint)                  # integer geometry bit-exact
     got = host(out)
-    assert_close(got, ref.out, "resample %s" % (shape,))
+    assert_close(got, ref.out, "resample %s" % (shape,), local=4)
     for k, (a, b) in enumerate(SHIFTS):                        # integer shifts are exact copies
         if a == np.floor(a) and b == np.floor(b):
             assert np.array_equal(got[k], ref.out[k])
@@ -333,7 +342,7 @@ def test_config1_full_size_stage_isolated():
     r = oracle.resample(c.out, -e.shift[:, 0], -e.shift[:, 1])
     reg, fp = mred.resample(dev(c.out), -e.shift[:, 0], -e.shift[:, 1])
     assert np.array_equal(fp, r.footprint)
-    assert_close(host(reg), r.out, "resample")
+    assert_close(host(reg), r.out, "resample", local=4)
     _compare_coadd(r.out, r.footprint, 0)
     _compare_coadd(r.out, r.footprint, 2)
 
@@ -348,7 +357,7 @@ def test_config4_stress_coadd_full_size():
     reg, fp = mred.resample(dev(c.out), sx, sy)
     # resample parity on a sample of frames (the oracle takes ~0.1 s per frame)
     r = oracle.resample(c.out[:4], sx[:4], sy[:4])
-    assert_close(host(reg)[:4], r.out, "resample cfg4")
+    assert_close(host(reg)[:4], r.out, "resample cfg4", local=4)
     st = host(reg)
     _compare_coadd(st, fp, 2)
 
