@@ -237,7 +237,7 @@ __device__ __forceinline__ void store_row(const Item& it, int y, int x, bool lan
     if (!lane_on) return;
     float* p = it.out + (size_t)y * it.w + x;
     if (VEC) {
-        if (x < it.w) *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+        *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);   // lane_on: x < w, and w % 4 == 0
         if (x + 4 < it.w) *reinterpret_cast<float4*>(p + 4) = make_float4(v[4], v[5], v[6], v[7]);
     } else {
 #pragma unroll
@@ -328,18 +328,55 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
     for (int y = max(yhi + 1, it.ya); y < it.yb; ++y) store_row<VEC>(it, y, yc.x0, yc.lane_on, fillv);
     if (ylo > yhi) return;
 
-    if (ax.ident && ay.ident) {     // pure integer translation: copy, 8 rows in flight per lane
-        for (int x = Xs + lane; x < Xe; x += 32) {
-            const bool ok = x >= ax.lo && x <= ax.hi;
-            const float* src = it.in + (size_t)ay.m * it.w + x + ax.m;
-            float* dst = it.out + x;
-            for (int y = ylo; y <= yhi; y += 8) {
-                float v[8];
+    if (ax.ident && ay.ident) {     // pure integer translation: copy with 16 independent loads in flight per lane
+        const int xa = max(Xs, ax.lo), xb = min(Xe - 1, ax.hi);       // columns that carry data (x_any: xa <= xb)
+        for (int y = ylo; y <= yhi; ++y) {                            // fill left and right of the footprint
+            float* dst = it.out + (size_t)y * it.w;
+            for (int x = Xs + lane; x < xa; x += 32) dst[x] = it.fill;
+            for (int x = xb + 1 + lane; x < Xe; x += 32) dst[x] = it.fill;
+        }
+        const int nrow = yhi - ylo + 1;
+        if (VEC && ((ax.m & 3) == 0) && ((xa & 3) == 0) && ((xb & 3) == 3)) {
+            const int c4 = (xb - xa + 1) >> 2, tot = c4 * nrow;
+            for (int base = 0; base < tot; base += 32 * 16) {
+                float4 v[16];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) v[i] = (ok && y + i <= yhi) ? __ldg(src + (size_t)(y + i) * it.w) : it.fill;
+                for (int i = 0; i < 16; ++i) {
+                    const int idx = base + lane + 32 * i;
+                    if (idx < tot) {
+                        const int yy = idx / c4, xx = xa + 4 * (idx - yy * c4);
+                        v[i] = __ldg(reinterpret_cast<const float4*>(it.in + (size_t)(ylo + yy + ay.m) * it.w + xx + ax.m));
+                    }
+                }
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (y + i <= yhi) dst[(size_t)(y + i) * it.w] = v[i];
+                for (int i = 0; i < 16; ++i) {
+                    const int idx = base + lane + 32 * i;
+                    if (idx < tot) {
+                        const int yy = idx / c4, xx = xa + 4 * (idx - yy * c4);
+                        *reinterpret_cast<float4*>(it.out + (size_t)(ylo + yy) * it.w + xx) = v[i];
+                    }
+                }
+            }
+        } else {
+            const int c1 = xb - xa + 1, tot = c1 * nrow;
+            for (int base = 0; base < tot; base += 32 * 16) {
+                float v[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const int idx = base + lane + 32 * i;
+                    if (idx < tot) {
+                        const int yy = idx / c1, xx = xa + (idx - yy * c1);
+                        v[i] = __ldg(it.in + (size_t)(ylo + yy + ay.m) * it.w + xx + ax.m);
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const int idx = base + lane + 32 * i;
+                    if (idx < tot) {
+                        const int yy = idx / c1, xx = xa + (idx - yy * c1);
+                        it.out[(size_t)(ylo + yy) * it.w + xx] = v[i];
+                    }
+                }
             }
         }
         return;
@@ -372,6 +409,7 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
     xf.pR = __any_sync(FULL, xf.r0 || xf.r1) ? it.w - 1 - (KC0 - r) : -1;
     if (xf.pL > WARPCOLS - 1) xf.pL = -1;         // column 0 not in the warp: no kept output needs the reflection
     if (xf.pR > WARPCOLS - 1 || it.w - 1 - (KC0 - r) < 0) xf.pR = -1;
+    const bool all_in = VEC && __all_sync(FULL, h0.mode == 0 && h1.mode == 0);
     float edge_row[V];                            // finished row 0 or h-1 (raw alignment), for the y reflection
     int edge_is = -1;
 #pragma unroll
@@ -406,7 +444,19 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
 #pragma unroll
             for (int j = 0; j < V; ++j) cur[i][j] = nxt[i][j];
 #pragma unroll
-        for (int i = 0; i < GR; ++i) load_row(it, row0 + GR + i, simple, h0, h1, nxt[i]);
+        if (all_in && row0 + GR >= 0 && row0 + 2 * GR <= it.h) {
+            const float4* p = reinterpret_cast<const float4*>(it.in + (size_t)(row0 + GR) * it.w + col_load);
+#pragma unroll
+            for (int i = 0; i < GR; ++i) {
+                const float4 a = __ldg(p), b = __ldg(p + 1);
+                nxt[i][0] = a.x; nxt[i][1] = a.y; nxt[i][2] = a.z; nxt[i][3] = a.w;
+                nxt[i][4] = b.x; nxt[i][5] = b.y; nxt[i][6] = b.z; nxt[i][7] = b.w;
+                p += it.w >> 2;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < GR; ++i) load_row(it, row0 + GR + i, simple, h0, h1, nxt[i]);
+        }
         if (gi < 0) continue;
         const int slot0 = (GR * gi) % (NRING * RB);
         if (simple) {
