@@ -4,7 +4,7 @@
 //
 //   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): float64 column
 //                partial sums per 64-row band and complete float64 row sums, valid-pixel counts.
-//   k_finalize : per (frame, axis): fixed-order band sum, mean, median by rank counting, subtract.
+//   k_finalize : per (frame, axis): fixed-order band sum, mean, median by a shared-memory bitonic sort, subtract.
 //   k_correlate: per (frame, axis): C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
 //                smaller |l| then smaller l; 3-point parabola.
 // No float atomics: every sum has a fixed order, so the integer result is reproducible.
@@ -12,7 +12,7 @@
 
 namespace mred {
 
-constexpr int PROF_BR = 64;        // rows per band
+constexpr int PROF_BR = 16;        // rows per band
 constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
 
 struct EstimateWs {
@@ -59,29 +59,44 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
         const int nv = max(0, min(4, w - x));
         double cs[4] = {0.0, 0.0, 0.0, 0.0};
         int cc[4] = {0, 0, 0, 0};
-        for (int y = y0; y < y1; ++y) {
-            float v[4] = {0.f, 0.f, 0.f, 0.f};
-            bool ok[4] = {false, false, false, false};
-            const size_t p = (size_t)y * w + x;
-            if (nv == 4 && vec_ok) {
-                const float4 t = __ldcs(reinterpret_cast<const float4*>(f + p));
-                v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
-                ok[0] = ok[1] = ok[2] = ok[3] = true;
-                if (bad) {
-                    const uchar4 b = __ldg(reinterpret_cast<const uchar4*>(bad + p));
-                    ok[0] = !b.x; ok[1] = !b.y; ok[2] = !b.z; ok[3] = !b.w;
-                }
-            } else {
-                for (int i = 0; i < nv; ++i) { v[i] = __ldcs(f + p + i); ok[i] = bad ? !__ldg(bad + p + i) : true; }
-            }
-            double rs = 0.0;
-            int rc = 0;
+        for (int yb = y0; yb < y1; yb += 4) {       // 4 rows in flight per thread
+            float v[4][4];
+            bool ok[4][4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (ok[i]) { const double d = (double)v[i]; cs[i] += d; ++cc[i]; rs += d; ++rc; }
-            rs = warp_sum(rs);
-            rc = warp_sum(rc);
-            if (lane == 0) { s_row[y - y0][warp] += rs; s_cnt[y - y0][warp] += rc; }
+            for (int u = 0; u < 4; ++u) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) { v[u][i] = 0.f; ok[u][i] = false; }
+                const int y = yb + u;
+                if (y >= y1) continue;
+                const size_t p = (size_t)y * w + x;
+                if (nv == 4 && vec_ok) {
+                    const float4 t = __ldcs(reinterpret_cast<const float4*>(f + p));
+                    v[u][0] = t.x; v[u][1] = t.y; v[u][2] = t.z; v[u][3] = t.w;
+                    ok[u][0] = ok[u][1] = ok[u][2] = ok[u][3] = true;
+                    if (bad) {
+                        const uchar4 b = __ldg(reinterpret_cast<const uchar4*>(bad + p));
+                        ok[u][0] = !b.x; ok[u][1] = !b.y; ok[u][2] = !b.z; ok[u][3] = !b.w;
+                    }
+                } else {
+                    for (int i = 0; i < nv; ++i) { v[u][i] = __ldcs(f + p + i); ok[u][i] = bad ? !__ldg(bad + p + i) : true; }
+                }
+            }
+            double rs[4] = {0.0, 0.0, 0.0, 0.0};
+            int rc[4] = {0, 0, 0, 0};
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (ok[u][i]) { const double d = (double)v[u][i]; cs[i] += d; ++cc[i]; rs[u] += d; ++rc[u]; }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { rs[u] += __shfl_xor_sync(0xffffffffu, rs[u], o); rc[u] += __shfl_xor_sync(0xffffffffu, rc[u], o); }
+            if (lane == 0) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (yb + u < y1) { s_row[yb + u - y0][warp] += rs[u]; s_cnt[yb + u - y0][warp] += rc[u]; }
+            }
         }
         for (int i = 0; i < nv; ++i) {
             e.colpart[((size_t)k * e.nbands + band) * w + x + i] = cs[i];
@@ -98,59 +113,69 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
     }
 }
 
-// grid (n, 2): axis 0 = x profile (length w), axis 1 = y profile (length h)
+// grid (n, 2): axis 0 = x profile (length w), axis 1 = y profile (length h).  Mean profile, then its median
+// by a bitonic sort in shared memory (invalid lines sort to the end as +inf), then the subtraction.
 __global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
 {
     __shared__ double s_p[PROF_MAXLEN];
-    __shared__ unsigned char s_ok[PROF_MAXLEN];
-    __shared__ double s_med[2];
     __shared__ int s_m;
     const int k = blockIdx.x, axis = blockIdx.y;
     const int len = axis == 0 ? w : h;
-    if (threadIdx.x == 0) { s_m = 0; s_med[0] = s_med[1] = 0.0; }
+    int P = 1;
+    while (P < len) P <<= 1;
+    if (threadIdx.x == 0) s_m = 0;
     __syncthreads();
-    int mymask = 0;
-    for (int i = threadIdx.x; i < len; i += blockDim.x) {
-        double s = 0.0;
-        int c = 0;
-        if (axis == 0) {
-            for (int b = 0; b < e.nbands; ++b) {
-                s += e.colpart[((size_t)k * e.nbands + b) * w + i];
-                c += e.colcnt[((size_t)k * e.nbands + b) * w + i];
-            }
-        } else {
-            s = e.rowsum[(size_t)k * h + i];
-            c = e.rowcnt[(size_t)k * h + i];
-        }
-        s_p[i] = c > 0 ? s / (double)c : 0.0;
-        s_ok[i] = c > 0;
-        mymask += c > 0;
-    }
-    if (mymask) atomicAdd(&s_m, mymask);
-    __syncthreads();
-    const int m = s_m;
-    if (m > 0) {
-        const int ia = (m - 1) >> 1, ib = m >> 1;
-        for (int i = threadIdx.x; i < len; i += blockDim.x) {
-            if (!s_ok[i]) continue;
-            const double vi = s_p[i];
-            int rank = 0;
-            for (int j = 0; j < len; ++j) {
-                const double vj = s_p[j];
-                rank += (s_ok[j] && (vj < vi || (vj == vi && j < i))) ? 1 : 0;
-            }
-            if (rank == ia) s_med[0] = vi;
-            if (rank == ib) s_med[1] = vi;
-        }
-    }
-    __syncthreads();
-    const double med = m > 0 ? ((m & 1) ? s_med[0] : 0.5 * (s_med[0] + s_med[1])) : 0.0;
     double* out = e.prof + ((size_t)k * 2 + axis) * e.plen;
-    for (int i = threadIdx.x; i < len; i += blockDim.x) out[i] = s_ok[i] ? s_p[i] - med : 0.0;
+    const double INF = __longlong_as_double(0x7ff0000000000000LL);
+    int mine = 0;
+    for (int i = threadIdx.x; i < P; i += blockDim.x) {
+        double v = INF;
+        if (i < len) {
+            double s = 0.0;
+            int c = 0;
+            if (axis == 0) {
+                for (int b = 0; b < e.nbands; ++b) {
+                    s += e.colpart[((size_t)k * e.nbands + b) * w + i];
+                    c += e.colcnt[((size_t)k * e.nbands + b) * w + i];
+                }
+            } else {
+                s = e.rowsum[(size_t)k * h + i];
+                c = e.rowcnt[(size_t)k * h + i];
+            }
+            if (c > 0) { v = s / (double)c; ++mine; }
+            out[i] = v;
+        }
+        s_p[i] = v;
+    }
+    if (mine) atomicAdd(&s_m, mine);
+    __syncthreads();
+    for (int kk = 2; kk <= P; kk <<= 1) {
+        for (int j = kk >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < P; i += blockDim.x) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const double a = s_p[i], b = s_p[l];
+                    const bool up = (i & kk) == 0;
+                    if ((a > b) == up) { s_p[i] = b; s_p[l] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+    const int m = s_m;
+    double med = 0.0;
+    if (m > 0) {
+        const double a = s_p[(m - 1) >> 1], b = s_p[m >> 1];
+        med = (m & 1) ? a : 0.5 * (a + b);
+    }
+    for (int i = threadIdx.x; i < len; i += blockDim.x) {
+        const double v = out[i];
+        out[i] = (v == INF) ? 0.0 : v - med;
+    }
 }
 
-// grid (n, 2), block 256
-__global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
+// grid (n, 2), block 1024: one lag per warp and round
+__global__ void __launch_bounds__(1024) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
                                                    int32_t* __restrict__ ishift, double* __restrict__ shift)
 {
     __shared__ double s_C[2 * MRED_MAX_LAG + 1];
@@ -163,7 +188,7 @@ __global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref,
     const double* a = e.prof + ((size_t)ref * 2 + axis) * e.plen;
     const double* b = e.prof + ((size_t)k * 2 + axis) * e.plen;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int l = -R + warp; l <= R; l += 8) {
+    for (int l = -R + warp; l <= R; l += 32) {
         const int j0 = max(0, -l), j1 = min(len, len - l);
         double s = 0.0;
         for (int j = j0 + lane; j < j1; j += 32) s = fma(a[j], b[j + l], s);
@@ -202,7 +227,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     MRED_LAUNCH_CHECK();
     k_finalize<<<dim3(n, 2), 1024, 0, st>>>(w, h, e);
     MRED_LAUNCH_CHECK();
-    k_correlate<<<dim3(n, 2), 256, 0, st>>>(w, h, n, ref, max_lag, e, ishift, shift);
+    k_correlate<<<dim3(n, 2), 1024, 0, st>>>(w, h, n, ref, max_lag, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
