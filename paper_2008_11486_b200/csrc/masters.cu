@@ -14,27 +14,29 @@
 namespace mred {
 
 struct MastersWs {            // layout of the caller's workspace (all 16-byte aligned)
-    unsigned long long* os_b; // [nb] overscan sums
-    unsigned long long* os_d; // [nd]
-    unsigned long long* os_f; // [nf]
+    unsigned long long* os;   // [nb + nd + nf] overscan sums (bias, dark, flat frames in that order)
     unsigned long long* img_f;// [nf] image-rectangle sums of the flats
+    unsigned int* ticket;     // [2] block counters of the two combine kernels (zeroed with the sums)
     double* part_bd;          // [nblocks][2] block sums of MB, MD
     double* part_f;           // [nblocks]    block sums of the un-normalised MF
     float* inv_gm;            // [nf] 1/<G_k>
     float* inv_mf;            // [1]  1/<MF_raw>
+    size_t zero_bytes;        // os, img_f, ticket are contiguous from os: one memset
     size_t bytes;
 };
+
+constexpr int MPX = 2;        // pixels per thread in the combine kernels (one 32-bit load per frame)
 
 static MastersWs carve(void* ws, const Geom& g, int nb, int nd, int nf)
 {
     MastersWs m;
     char* p = static_cast<char*>(ws);
     auto take = [&](size_t b) { char* q = p; p += align_up(b, 16); return q; };
-    const size_t nblocks = ((size_t)g.w * g.h + 255) / 256;
-    m.os_b = reinterpret_cast<unsigned long long*>(take(8 * (size_t)nb));
-    m.os_d = reinterpret_cast<unsigned long long*>(take(8 * (size_t)nd));
-    m.os_f = reinterpret_cast<unsigned long long*>(take(8 * (size_t)nf));
+    const size_t nblocks = ((size_t)g.w * g.h + 255) / 256;     // upper bound for either pixels-per-thread
+    m.os = reinterpret_cast<unsigned long long*>(take(8 * (size_t)(nb + nd + nf)));
     m.img_f = reinterpret_cast<unsigned long long*>(take(8 * (size_t)nf));
+    m.ticket = reinterpret_cast<unsigned int*>(take(16));
+    m.zero_bytes = (size_t)(p - static_cast<char*>(ws));
     m.part_bd = reinterpret_cast<double*>(take(16 * nblocks));
     m.part_f = reinterpret_cast<double*>(take(8 * nblocks));
     m.inv_gm = reinterpret_cast<float*>(take(4 * (size_t)nf));
@@ -46,6 +48,46 @@ static MastersWs carve(void* ws, const Geom& g, int nb, int nd, int nf)
 size_t masters_ws_bytes(const Geom& g, int n)
 {
     return carve(nullptr, g, n, n, n).bytes;   // n = max(nb, nd, nf) is an upper bound for each
+}
+
+// Exact integer sums of all three stacks in one launch: overscan columns of every frame, and the image
+// rectangle of the flats (for <F_k>).  grid (row_chunks, nb+nd+nf), block 256; integer atomics -> bit-exact.
+constexpr int MSUM_ROWS = 32;
+__global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict__ bias, int nb,
+                                                     const uint16_t* __restrict__ dark, int nd,
+                                                     const uint16_t* __restrict__ flat, int nf, Geom g,
+                                                     unsigned long long* __restrict__ os,
+                                                     unsigned long long* __restrict__ img_f, int pair_ok)
+{
+    const int k = blockIdx.y;
+    const size_t fs = (size_t)g.W * g.H;
+    const uint16_t* f = k < nb ? bias + (size_t)k * fs : (k < nb + nd ? dark + (size_t)(k - nb) * fs : flat + (size_t)(k - nb - nd) * fs);
+    const bool want_img = k >= nb + nd;
+    const int r0 = blockIdx.x * MSUM_ROWS;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned long long s_os = 0, s_img = 0;
+    for (int r = r0 + warp; r < min(r0 + MSUM_ROWS, g.H); r += 8) {
+        const uint16_t* row = f + (size_t)r * g.W;
+        unsigned int a = 0;
+        for (int x = g.os_x0 + lane; x < g.os_x1; x += 32) a += __ldg(row + x);
+        s_os += a;
+        if (want_img && r >= g.y0 && r < g.y0 + g.h) {
+            unsigned long long b = 0;
+            if (pair_ok) {      // two pixels per 32-bit load
+                const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
+                for (int x = lane; x < (g.w >> 1); x += 32) { const unsigned int v = __ldg(row2 + x); b += (v & 0xffffu) + (v >> 16); }
+            } else {
+                for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
+            }
+            s_img += b;
+        }
+    }
+    s_os = warp_sum(s_os);
+    if (lane == 0 && s_os) atomicAdd(os + k, s_os);
+    if (want_img) {
+        s_img = warp_sum(s_img);
+        if (lane == 0 && s_img) atomicAdd(img_f + (k - nb - nd), s_img);
+    }
 }
 
 // deterministic block sum of one double per thread (256 threads): shuffle tree, then warp 0 adds the
@@ -69,152 +111,215 @@ __device__ __forceinline__ float combine_all(float (&v)[NMAX], int n, float ksig
     return combine_mean_clip<NMAX>(v, n, MODE == MRED_SIGCLIP, ksigma, max_iter).value;
 }
 
-// ---- bias + dark ----------------------------------------------------------------------------
-template <int NMAX, int MODE>
+// PX pixels of frame k starting at element q of the frame (PX = 2: one aligned 32-bit load)
+template <int PX>
+__device__ __forceinline__ void load_px(const uint16_t* f, size_t q, int nv, float (&o)[PX])
+{
+    if (PX == 2) {
+        const unsigned int v = __ldcs(reinterpret_cast<const unsigned int*>(f + q));
+        o[0] = (float)(v & 0xffffu); o[PX - 1] = (float)(v >> 16);
+    } else {
+#pragma unroll
+        for (int i = 0; i < PX; ++i) o[i] = i < nv ? (float)__ldcs(f + q + i) : 0.f;
+    }
+}
+
+// true in exactly one block: the last one to arrive (its reads of the other blocks' partial sums are ordered
+// by the fence / atomic pair)
+__device__ __forceinline__ bool last_block(unsigned int* ticket)
+{
+    __shared__ int s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    return s_last != 0;
+}
+
+// ---- bias + dark; the last block turns the block sums into 1/<G_k> of every flat ----------------
+template <int NMAX, int MODE, int PX>
 __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__ bias, int nb,
-                                                    const uint16_t* __restrict__ dark, int nd, Geom g,
-                                                    const unsigned long long* __restrict__ os_b,
-                                                    const unsigned long long* __restrict__ os_d, float ksigma,
-                                                    int max_iter, float* __restrict__ MB, float* __restrict__ MD,
-                                                    double* __restrict__ part_bd)
+                                                    const uint16_t* __restrict__ dark, int nd, int nf, Geom g,
+                                                    MastersWs m, double r, float ksigma, int max_iter,
+                                                    float* __restrict__ MB, float* __restrict__ MD)
 {
     __shared__ float s_lb[MRED_MAX_STACK + 1], s_ld[MRED_MAX_STACK + 1];
     __shared__ double s8[8];
-    const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
-    for (int k = threadIdx.x; k < nb; k += blockDim.x) s_lb[k] = cnt > 0 ? (float)((double)os_b[k] / (double)cnt) : 0.f;
-    for (int k = threadIdx.x; k < nd; k += blockDim.x) s_ld[k] = cnt > 0 ? (float)((double)os_d[k] / (double)cnt) : 0.f;
-    __syncthreads();
-    const size_t np = (size_t)g.w * g.h, fs = (size_t)g.W * g.H;
-    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = p < np;
-    const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
-    float mb = 0.f, md = 0.f;
-    if (live) {
-        const int y = (int)(p / g.w), x = (int)(p - (size_t)y * g.w);
-        const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
-        float v[NMAX];
-#pragma unroll
-        for (int k = 0; k < NMAX; ++k) v[k] = k < nb ? (float)__ldcs(bias + (size_t)k * fs + q) - s_lb[k] : ABSENT;
-        mb = combine_all<NMAX, MODE>(v, nb, ksigma, max_iter);
-#pragma unroll
-        for (int k = 0; k < NMAX; ++k)
-            v[k] = k < nd ? ((float)__ldcs(dark + (size_t)k * fs + q) - s_ld[k]) - mb : ABSENT;
-        md = combine_all<NMAX, MODE>(v, nd, ksigma, max_iter);
-        MB[p] = mb;
-        MD[p] = md;
-    }
-    const double sb = block_sum_256((double)mb, s8);
-    const double sd = block_sum_256((double)md, s8);
-    if (threadIdx.x == 0) { part_bd[2 * (size_t)blockIdx.x] = sb; part_bd[2 * (size_t)blockIdx.x + 1] = sd; }
-}
-
-// ---- <G_k> from the sums (one block) -----------------------------------------------------------
-__global__ void __launch_bounds__(256) k_flat_means(const double* __restrict__ part_bd, int nblocks, Geom g, int nf,
-                                                    const unsigned long long* __restrict__ os_f,
-                                                    const unsigned long long* __restrict__ img_f, double r,
-                                                    float* __restrict__ inv_gm)
-{
-    __shared__ double s8[8];
     __shared__ double s_mean[2];
-    double a = 0.0, b = 0.0;
-    for (int i = threadIdx.x; i < nblocks; i += blockDim.x) { a += part_bd[2 * (size_t)i]; b += part_bd[2 * (size_t)i + 1]; }
-    const double sa = block_sum_256(a, s8);
-    const double sb = block_sum_256(b, s8);
-    const double np = (double)g.w * (double)g.h;
-    if (threadIdx.x == 0) { s_mean[0] = sa / np; s_mean[1] = sb / np; }
-    __syncthreads();
     const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
+    for (int k = threadIdx.x; k < nb; k += blockDim.x) s_lb[k] = cnt > 0 ? (float)((double)m.os[k] / (double)cnt) : 0.f;
+    for (int k = threadIdx.x; k < nd; k += blockDim.x) s_ld[k] = cnt > 0 ? (float)((double)m.os[nb + k] / (double)cnt) : 0.f;
+    __syncthreads();
+    const size_t fs = (size_t)g.W * g.H;
+    const int wg = (g.w + PX - 1) / PX;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
+    float mb[PX], md[PX];
+#pragma unroll
+    for (int i = 0; i < PX; ++i) { mb[i] = 0.f; md[i] = 0.f; }
+    if (gid < (long long)g.h * wg) {
+        const int y = (int)(gid / wg), x = (int)(gid - (long long)y * wg) * PX;
+        const int nv = min(PX, g.w - x);
+        const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
+        const size_t p = (size_t)y * g.w + x;
+        float v[PX][NMAX];
+#pragma unroll
+        for (int k = 0; k < NMAX; ++k) {
+            float o[PX];
+            if (k < nb) load_px<PX>(bias + (size_t)k * fs, q, nv, o);
+#pragma unroll
+            for (int i = 0; i < PX; ++i) v[i][k] = k < nb ? o[i] - s_lb[k] : ABSENT;
+        }
+#pragma unroll
+        for (int i = 0; i < PX; ++i) mb[i] = combine_all<NMAX, MODE>(v[i], nb, ksigma, max_iter);
+#pragma unroll
+        for (int k = 0; k < NMAX; ++k) {
+            float o[PX];
+            if (k < nd) load_px<PX>(dark + (size_t)k * fs, q, nv, o);
+#pragma unroll
+            for (int i = 0; i < PX; ++i) v[i][k] = k < nd ? (o[i] - s_ld[k]) - mb[i] : ABSENT;
+        }
+#pragma unroll
+        for (int i = 0; i < PX; ++i) md[i] = combine_all<NMAX, MODE>(v[i], nd, ksigma, max_iter);
+        if (PX == 2) {
+            *reinterpret_cast<float2*>(MB + p) = make_float2(mb[0], mb[PX - 1]);
+            *reinterpret_cast<float2*>(MD + p) = make_float2(md[0], md[PX - 1]);
+        } else {
+            for (int i = 0; i < nv; ++i) { MB[p + i] = mb[i]; MD[p + i] = md[i]; }
+        }
+#pragma unroll
+        for (int i = 0; i < PX; ++i)
+            if (i >= nv) { mb[i] = 0.f; md[i] = 0.f; }
+    }
+    double tb = 0.0, td = 0.0;
+#pragma unroll
+    for (int i = 0; i < PX; ++i) { tb += (double)mb[i]; td += (double)md[i]; }
+    const double sb = block_sum_256(tb, s8);
+    const double sd = block_sum_256(td, s8);
+    if (threadIdx.x == 0) { m.part_bd[2 * (size_t)blockIdx.x] = sb; m.part_bd[2 * (size_t)blockIdx.x + 1] = sd; }
+    if (!last_block(m.ticket)) return;
+    // <G_k> = <F_k> - L_k - <MB> - r <MD>: fixed-order sums of the block partials
+    double a = 0.0, b = 0.0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) { a += __ldcg(m.part_bd + 2 * (size_t)i); b += __ldcg(m.part_bd + 2 * (size_t)i + 1); }
+    const double sa = block_sum_256(a, s8);
+    const double sbb = block_sum_256(b, s8);
+    const double np = (double)g.w * (double)g.h;
+    if (threadIdx.x == 0) { s_mean[0] = sa / np; s_mean[1] = sbb / np; }
+    __syncthreads();
     for (int k = threadIdx.x; k < nf; k += blockDim.x) {
-        const double L = cnt > 0 ? (double)os_f[k] / (double)cnt : 0.0;
-        const double gm = (double)img_f[k] / np - L - s_mean[0] - r * s_mean[1];
-        inv_gm[k] = (float)(1.0 / gm);
+        const double L = cnt > 0 ? (double)m.os[nb + nd + k] / (double)cnt : 0.0;
+        const double gm = (double)m.img_f[k] / np - L - s_mean[0] - r * s_mean[1];
+        m.inv_gm[k] = (float)(1.0 / gm);
     }
 }
 
-// ---- flat -----------------------------------------------------------------------------------
-template <int NMAX, int MODE>
-__global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ flat, int nf, Geom g,
-                                                   const unsigned long long* __restrict__ os_f,
-                                                   const float* __restrict__ inv_gm, float r, float ksigma, int max_iter,
+// ---- flat; the last block turns the block sums into 1/<MF_raw> ---------------------------------
+template <int NMAX, int MODE, int PX>
+__global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ flat, int nb, int nd, int nf, Geom g,
+                                                   MastersWs m, float r, float ksigma, int max_iter,
                                                    const float* __restrict__ MB, const float* __restrict__ MD,
-                                                   float* __restrict__ MF, double* __restrict__ part_f)
+                                                   float* __restrict__ MF)
 {
     __shared__ float s_lf[MRED_MAX_STACK + 1], s_ig[MRED_MAX_STACK + 1];
     __shared__ double s8[8];
     const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
     for (int k = threadIdx.x; k < nf; k += blockDim.x) {
-        s_lf[k] = cnt > 0 ? (float)((double)os_f[k] / (double)cnt) : 0.f;
-        s_ig[k] = inv_gm[k];
+        s_lf[k] = cnt > 0 ? (float)((double)m.os[nb + nd + k] / (double)cnt) : 0.f;
+        s_ig[k] = m.inv_gm[k];
     }
     __syncthreads();
-    const size_t np = (size_t)g.w * g.h, fs = (size_t)g.W * g.H;
-    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t fs = (size_t)g.W * g.H;
+    const int wg = (g.w + PX - 1) / PX;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
-    float mf = 0.f;
-    if (p < np) {
-        const int y = (int)(p / g.w), x = (int)(p - (size_t)y * g.w);
-        const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
-        const float off = fmaf(r, MD[p], MB[p]);
-        float v[NMAX];
+    float mf[PX];
 #pragma unroll
-        for (int k = 0; k < NMAX; ++k)
-            v[k] = k < nf ? (((float)__ldg(flat + (size_t)k * fs + q) - s_lf[k]) - off) * s_ig[k] : ABSENT;
-        mf = combine_all<NMAX, MODE>(v, nf, ksigma, max_iter);
-        MF[p] = mf;
+    for (int i = 0; i < PX; ++i) mf[i] = 0.f;
+    if (gid < (long long)g.h * wg) {
+        const int y = (int)(gid / wg), x = (int)(gid - (long long)y * wg) * PX;
+        const int nv = min(PX, g.w - x);
+        const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
+        const size_t p = (size_t)y * g.w + x;
+        float off[PX];
+#pragma unroll
+        for (int i = 0; i < PX; ++i) off[i] = i < nv ? fmaf(r, MD[p + i], MB[p + i]) : 0.f;
+        float v[PX][NMAX];
+#pragma unroll
+        for (int k = 0; k < NMAX; ++k) {
+            float o[PX];
+            if (k < nf) load_px<PX>(flat + (size_t)k * fs, q, nv, o);
+#pragma unroll
+            for (int i = 0; i < PX; ++i) v[i][k] = k < nf ? ((o[i] - s_lf[k]) - off[i]) * s_ig[k] : ABSENT;
+        }
+#pragma unroll
+        for (int i = 0; i < PX; ++i) mf[i] = combine_all<NMAX, MODE>(v[i], nf, ksigma, max_iter);
+        if (PX == 2) *reinterpret_cast<float2*>(MF + p) = make_float2(mf[0], mf[PX - 1]);
+        else for (int i = 0; i < nv; ++i) MF[p + i] = mf[i];
+#pragma unroll
+        for (int i = 0; i < PX; ++i)
+            if (i >= nv) mf[i] = 0.f;
     }
-    const double s = block_sum_256((double)mf, s8);
-    if (threadIdx.x == 0) part_f[blockIdx.x] = s;
-}
-
-__global__ void __launch_bounds__(256) k_mf_mean(const double* __restrict__ part_f, int nblocks, double np,
-                                                 float* __restrict__ inv_mf)
-{
-    __shared__ double s8[8];
+    double t = 0.0;
+#pragma unroll
+    for (int i = 0; i < PX; ++i) t += (double)mf[i];
+    const double sblk = block_sum_256(t, s8);
+    if (threadIdx.x == 0) m.part_f[blockIdx.x] = sblk;
+    if (!last_block(m.ticket + 1)) return;
     double a = 0.0;
-    for (int i = threadIdx.x; i < nblocks; i += blockDim.x) a += part_f[i];
-    const double s = block_sum_256(a, s8);
-    if (threadIdx.x == 0) inv_mf[0] = (float)(np / s);
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) a += __ldcg(m.part_f + i);
+    const double sall = block_sum_256(a, s8);
+    if (threadIdx.x == 0) m.inv_mf[0] = (float)((double)g.w * (double)g.h / sall);
 }
 
-__global__ void __launch_bounds__(256) k_mf_scale(float* __restrict__ MF, size_t np, const float* __restrict__ inv_mf)
+__global__ void __launch_bounds__(256) k_mf_scale(float* __restrict__ MF, size_t np, const float* __restrict__ inv_mf, int vec)
 {
-    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p < np) MF[p] *= inv_mf[0];
+    const float sc = inv_mf[0];
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vec) {
+        if (4 * i + 3 < np) {
+            float4 v = reinterpret_cast<float4*>(MF)[i];
+            v.x *= sc; v.y *= sc; v.z *= sc; v.w *= sc;
+            reinterpret_cast<float4*>(MF)[i] = v;
+        }
+    } else {
+        for (size_t p = 4 * i; p < np && p < 4 * i + 4; ++p) MF[p] *= sc;
+    }
 }
 
-template <int NMAX>
+template <int NMAX, int PX>
 static void launch_bd(int mode, dim3 grid, cudaStream_t st, const uint16_t* bias, int nb, const uint16_t* dark, int nd,
-                      const Geom& g, const MastersWs& m, float ks, int mi, float* MB, float* MD)
+                      int nf, const Geom& g, const MastersWs& m, double r, float ks, int mi, float* MB, float* MD)
 {
     if (mode == MRED_MEDIAN)
-        k_masters_bd<NMAX, MRED_MEDIAN><<<grid, 256, 0, st>>>(bias, nb, dark, nd, g, m.os_b, m.os_d, ks, mi, MB, MD, m.part_bd);
+        k_masters_bd<NMAX, MRED_MEDIAN, PX><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
     else if (mode == MRED_MEAN)
-        k_masters_bd<NMAX, MRED_MEAN><<<grid, 256, 0, st>>>(bias, nb, dark, nd, g, m.os_b, m.os_d, ks, mi, MB, MD, m.part_bd);
+        k_masters_bd<NMAX, MRED_MEAN, PX><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
     else
-        k_masters_bd<NMAX, MRED_SIGCLIP><<<grid, 256, 0, st>>>(bias, nb, dark, nd, g, m.os_b, m.os_d, ks, mi, MB, MD, m.part_bd);
+        k_masters_bd<NMAX, MRED_SIGCLIP, PX><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
 }
 
-template <int NMAX>
-static void launch_f(int mode, dim3 grid, cudaStream_t st, const uint16_t* flat, int nf, const Geom& g,
+template <int NMAX, int PX>
+static void launch_f(int mode, dim3 grid, cudaStream_t st, const uint16_t* flat, int nb, int nd, int nf, const Geom& g,
                      const MastersWs& m, float r, float ks, int mi, const float* MB, const float* MD, float* MF)
 {
     if (mode == MRED_MEDIAN)
-        k_masters_f<NMAX, MRED_MEDIAN><<<grid, 256, 0, st>>>(flat, nf, g, m.os_f, m.inv_gm, r, ks, mi, MB, MD, MF, m.part_f);
+        k_masters_f<NMAX, MRED_MEDIAN, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
     else if (mode == MRED_MEAN)
-        k_masters_f<NMAX, MRED_MEAN><<<grid, 256, 0, st>>>(flat, nf, g, m.os_f, m.inv_gm, r, ks, mi, MB, MD, MF, m.part_f);
+        k_masters_f<NMAX, MRED_MEAN, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
     else
-        k_masters_f<NMAX, MRED_SIGCLIP><<<grid, 256, 0, st>>>(flat, nf, g, m.os_f, m.inv_gm, r, ks, mi, MB, MD, MF, m.part_f);
+        k_masters_f<NMAX, MRED_SIGCLIP, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
 }
 
-#define MRED_BUCKET(n, CALL)                 \
-    do {                                     \
-        if ((n) <= 4) { CALL(4); }           \
-        else if ((n) <= 8) { CALL(8); }      \
-        else if ((n) <= 16) { CALL(16); }    \
-        else if ((n) <= 32) { CALL(32); }    \
-        else if ((n) <= 64) { CALL(64); }    \
-        else if ((n) <= 128) { CALL(128); }  \
-        else { CALL(256); }                  \
+// capacity buckets; two pixels per thread up to 32 frames (register budget), one above
+#define MRED_BUCKET(n, CALL)                     \
+    do {                                         \
+        if ((n) <= 4) { CALL(4, 2); }            \
+        else if ((n) <= 8) { CALL(8, 2); }       \
+        else if ((n) <= 16) { CALL(16, 2); }     \
+        else if ((n) <= 32) { CALL(32, 2); }     \
+        else if ((n) <= 64) { CALL(64, 1); }     \
+        else if ((n) <= 128) { CALL(128, 1); }   \
+        else { CALL(256, 1); }                   \
     } while (0)
 
 int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint16_t* dark, int nd, float t_dark,
@@ -222,28 +327,34 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
                          float* MF, void* ws, cudaStream_t st)
 {
     const MastersWs m = carve(ws, g, nb, nd, nf);
-    int rc;
-    if ((rc = launch_frame_sums(bias, g, nb, m.os_b, nullptr, st))) return rc;
-    if ((rc = launch_frame_sums(dark, g, nd, m.os_d, nullptr, st))) return rc;
-    if ((rc = launch_frame_sums(flat, g, nf, m.os_f, m.img_f, st))) return rc;
+    MRED_CUDA_TRY(cudaMemsetAsync(m.os, 0, m.zero_bytes, st));
+    // pairs of pixels by one 32-bit load need even W, x0 and w (frame bases are 16-byte aligned, frames W*H*2 B)
+    const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0 && g.w % 2 == 0 && ((size_t)g.W * g.H) % 2 == 0) ? 1 : 0;
+    k_master_sums<<<dim3((g.H + MSUM_ROWS - 1) / MSUM_ROWS, nb + nd + nf), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, m.os,
+                                                                                     m.img_f, pair_ok);
+    MRED_LAUNCH_CHECK();
     const size_t np = (size_t)g.w * g.h;
-    const int nblocks = (int)((np + 255) / 256);
-    dim3 grid(nblocks);
     const int nbd = nb > nd ? nb : nd;
     const float r = t_flat / t_dark;
-#define CALL_BD(N) launch_bd<N>(o.mode, grid, st, bias, nb, dark, nd, g, m, o.ksigma, o.max_iter, MB, MD)
+    const double rd = (double)t_flat / (double)t_dark;
+#define CALL_BD(N, PX)                                                                                         \
+    do {                                                                                                       \
+        if (PX == 2 && pair_ok) launch_bd<N, PX>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        else launch_bd<N, 1>(o.mode, dim3((unsigned)((np + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+    } while (0)
     MRED_BUCKET(nbd, CALL_BD);
 #undef CALL_BD
     MRED_LAUNCH_CHECK();
-    k_flat_means<<<1, 256, 0, st>>>(m.part_bd, nblocks, g, nf, m.os_f, m.img_f, (double)t_flat / (double)t_dark, m.inv_gm);
-    MRED_LAUNCH_CHECK();
-#define CALL_F(N) launch_f<N>(o.mode, grid, st, flat, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF)
+#define CALL_F(N, PX)                                                                                          \
+    do {                                                                                                       \
+        if (PX == 2 && pair_ok) launch_f<N, PX>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        else launch_f<N, 1>(o.mode, dim3((unsigned)((np + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+    } while (0)
     MRED_BUCKET(nf, CALL_F);
 #undef CALL_F
     MRED_LAUNCH_CHECK();
-    k_mf_mean<<<1, 256, 0, st>>>(m.part_f, nblocks, (double)np, m.inv_mf);
-    MRED_LAUNCH_CHECK();
-    k_mf_scale<<<grid, 256, 0, st>>>(MF, np, m.inv_mf);
+    const int vec = (np % 4 == 0) ? 1 : 0;
+    k_mf_scale<<<dim3((unsigned)((np + 1023) / 1024)), 256, 0, st>>>(MF, np, m.inv_mf, vec);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
