@@ -16,26 +16,63 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
                                                float* __restrict__ out, uint16_t* __restrict__ count,
                                                uint32_t* __restrict__ rejmask)
 {
+    constexpr int NW = (NMAX + 31) / 32;
+    __shared__ int4 s_fp[NMAX];
+    __shared__ uint32_t s_in[NW], s_part[NW];
     const size_t np = (size_t)w * h;
+    // Classify every frame against the block's 256 consecutive pixels: footprint covers all of them (the
+    // usual case: bit in s_in, no per-pixel test), none of them, or some (bit in s_part: per-pixel test).
+    {
+        const size_t p0 = (size_t)blockIdx.x * blockDim.x;
+        const size_t p1 = min(p0 + blockDim.x, np) - 1;
+        const int ya = (int)(p0 / w), yb = (int)(p1 / w);
+        const int xa = (int)(p0 - (size_t)ya * w), xb = (int)(p1 - (size_t)yb * w);
+        const int k = threadIdx.x;
+        if (k < NW * 32) {
+            int cls = 0;                                   // 0 none, 1 all, 2 some
+            if (k < n) {
+                int4 f = make_int4(0, w - 1, 0, h - 1);
+                if (use_fp) f = fp_dev ? fp_dev[k] : hfp.fp[k];
+                if (k < NMAX) s_fp[k] = f;
+                const bool rows_in = ya >= f.z && yb <= f.w, rows_out = yb < f.z || ya > f.w || f.x > f.y;
+                if (ya == yb) {
+                    const bool cols_in = xa >= f.x && xb <= f.y, cols_out = xb < f.x || xa > f.y;
+                    cls = (rows_in && cols_in) ? 1 : ((rows_out || cols_out) ? 0 : 2);
+                } else {
+                    cls = (rows_in && f.x <= 0 && f.y >= w - 1) ? 1 : (rows_out ? 0 : 2);
+                }
+            }
+            const uint32_t bin = __ballot_sync(0xffffffffu, cls == 1), bpart = __ballot_sync(0xffffffffu, cls == 2);
+            if ((k & 31) == 0) { s_in[k >> 5] = bin; s_part[k >> 5] = bpart; }
+        }
+        __syncthreads();
+    }
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
     const int y = (int)(p / w), x = (int)(p - (size_t)y * w);
-    const int4* fp = fp_dev ? fp_dev : hfp.fp;
     const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
     float v[NMAX];
-    uint32_t inside[(NMAX + 31) / 32];
+    uint32_t inside[NW];
 #pragma unroll
-    for (int i = 0; i < (NMAX + 31) / 32; ++i) inside[i] = 0u;
+    for (int i = 0; i < NW; ++i) inside[i] = s_in[i];
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+        uint32_t part = s_part[i];
+        while (part) {                                     // block-uniform, rarely non-zero
+            const int b = __ffs(part) - 1;
+            part &= part - 1;
+            const int4 f = s_fp[32 * i + b];
+            if (x >= f.x && x <= f.y && y >= f.z && y <= f.w) inside[i] |= 1u << b;
+        }
+    }
     int m = 0;
 #pragma unroll
+    for (int i = 0; i < NW; ++i) m += __popc(inside[i]);
+    const float* src = stack + p;
+#pragma unroll
     for (int k = 0; k < NMAX; ++k) {
-        bool ok = k < n;
-        if (use_fp && ok) {
-            const int4 f = fp[k];
-            ok = (x >= f.x) && (x <= f.y) && (y >= f.z) && (y <= f.w);
-        }
-        v[k] = ok ? __ldcs(stack + (size_t)k * np + p) : ABSENT;
-        if (ok) { ++m; inside[k >> 5] |= 1u << (k & 31); }
+        const bool ok = (inside[k >> 5] >> (k & 31)) & 1u;
+        v[k] = ok ? __ldcs(src + (size_t)k * np) : ABSENT;
     }
     Combined r;
     uint32_t rej[(NMAX + 31) / 32];
@@ -176,11 +213,22 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
     const int mi = o.max_iter;
     if (n <= 128) {
         dim3 grid((unsigned)((np + 255) / 256));
-        if (n <= 8) launch_mode<8>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
-        else if (n <= 16) launch_mode<16>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
-        else if (n <= 32) launch_mode<32>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
-        else if (n <= 64) launch_mode<64>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
-        else launch_mode<128>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
+#define MRED_CO(N) launch_mode<N>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask)
+        if (n <= 4) MRED_CO(4);
+        else if (n <= 5) MRED_CO(5);
+        else if (n <= 8) MRED_CO(8);
+        else if (n <= 10) MRED_CO(10);
+        else if (n <= 12) MRED_CO(12);
+        else if (n <= 16) MRED_CO(16);
+        else if (n <= 20) MRED_CO(20);
+        else if (n <= 24) MRED_CO(24);
+        else if (n <= 32) MRED_CO(32);
+        else if (n <= 48) MRED_CO(48);
+        else if (n <= 60) MRED_CO(60);
+        else if (n <= 64) MRED_CO(64);
+        else if (n <= 100) MRED_CO(100);
+        else MRED_CO(128);
+#undef MRED_CO
     } else {
         dim3 grid((unsigned)((np + 127) / 128));
         if (o.mode == MRED_MEDIAN)

@@ -108,6 +108,11 @@ __device__ __forceinline__ Combined combine_mean_clip(float (&v)[NMAX], int m, b
             // + 1e-10|c|: identical inputs give S = 0 while t carries a few ulp(d) of rounding from the
             // running sums; the slack (1e-7 ADU at 1000 ADU) keeps them, and is far below any tie margin
             const float thr = fmaf(ksigma, sqrtf(S / (float)cnt), 1e-10f * fabsf(c));
+            // cheap look first: most columns lose nothing in a pass (NaN compares false: absent entries never count)
+            bool any = false;
+#pragma unroll
+            for (int i = 0; i < NMAX; ++i) any = any || (fabsf(v[i] - mean) > thr);
+            if (!any) break;
             float n1 = 0.f, n2 = 0.f;
             int ncnt = 0;
 #pragma unroll

@@ -310,13 +310,22 @@ static void launch_f(int mode, dim3 grid, cudaStream_t st, const uint16_t* flat,
         k_masters_f<NMAX, MRED_SIGCLIP, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
 }
 
-// capacity buckets; two pixels per thread up to 32 frames (register budget), one above
+// capacity buckets (the sorting network and every sweep are unrolled over the capacity, so a tight bucket
+// is a direct saving); two pixels per thread up to 32 frames (register budget), one above
 #define MRED_BUCKET(n, CALL)                     \
     do {                                         \
-        if ((n) <= 4) { CALL(4, 2); }            \
+        if ((n) <= 3) { CALL(3, 2); }            \
+        else if ((n) <= 4) { CALL(4, 2); }       \
+        else if ((n) <= 5) { CALL(5, 2); }       \
+        else if ((n) <= 6) { CALL(6, 2); }       \
         else if ((n) <= 8) { CALL(8, 2); }       \
+        else if ((n) <= 10) { CALL(10, 2); }     \
+        else if ((n) <= 12) { CALL(12, 2); }     \
         else if ((n) <= 16) { CALL(16, 2); }     \
+        else if ((n) <= 20) { CALL(20, 2); }     \
+        else if ((n) <= 24) { CALL(24, 2); }     \
         else if ((n) <= 32) { CALL(32, 2); }     \
+        else if ((n) <= 48) { CALL(48, 1); }     \
         else if ((n) <= 64) { CALL(64, 1); }     \
         else if ((n) <= 128) { CALL(128, 1); }   \
         else { CALL(256, 1); }                   \
