@@ -8,6 +8,7 @@ One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for what each key
 from __future__ import annotations
 
 import argparse
+import contextlib
 import json
 import os
 import subprocess
@@ -36,6 +37,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default: configs[1])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--streams", type=int, default=0, help="CUDA streams the groups are spread over (0 = one per group)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -69,44 +71,52 @@ def stage_bytes(g, n, nm, want_mask_words=0):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled DURING the timed region (B200_PROFILING.md): NVML polled from a
+    thread every ~1 ms (the timed region of the small configs lasts milliseconds, too short for nvidia-smi -lms)."""
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.index, self.rows, self.stop_flag, self.h, self.t = index, [], False, None, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+        except Exception:
+            self.nv = None
+
+    def _poll(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.rows.append((sm, rs))
+            except Exception:
+                break
+            time.sleep(0.001)
 
     def start(self):
-        try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
-        except OSError:
-            self.proc = None
-
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+        if self.nv is None:
+            return
+        self.t = threading.Thread(target=self._poll, daemon=True)
+        self.t.start()
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
+        if self.nv is None or self.t is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"], "samples": 0}
+        self.stop_flag = True
         self.t.join(timeout=2)
-        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
-        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
-        reasons = set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
-            if len(r) >= 9:
-                for nm, v in zip(names, r[5:9]):
-                    if v.lower().startswith("active"):
-                        reasons.add(nm)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+        nv = self.nv
+        mx = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake_slowdown": 0x80}
+        reasons = sorted(k for k, bit in names.items() if any(r & bit for _, r in self.rows))
+        sm = [r[0] for r in self.rows]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(mx), "reasons": reasons,
+                "samples": len(sm)}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -214,18 +224,38 @@ def run_ours(args):
     scale = groups[0].t_sci / groups[0].t_dark
     nstage = len(STAGES)
 
+    # groups are independent: each runs on its own stream, so that the small per-group kernels of different
+    # groups overlap; a step starts and ends on the current stream (fork / join by events)
+    nstreams = G if args.streams <= 0 else min(args.streams, G)
+    streams = [torch.cuda.Stream(device=devs) for _ in range(nstreams)] if nstreams > 1 else [None]
+    mwss = [torch.empty_like(mws) for _ in streams]
+    masters_out = [None] * G
+
     def step(ev_m, ev_s):
         """One pass of the whole hot path over the batch: every group, masters then the chained science path."""
+        main = torch.cuda.current_stream()
+        fork = torch.cuda.Event()
+        fork.record(main)
         for gi in range(G):
+            st = streams[gi % len(streams)]
             d = devg[gi]
-            if ev_m is not None:
-                ev_m[gi][0].record()
-            MB, MD, MF = mred.build_masters(g, d["bias"], d["dark"], groups[gi].t_dark, d["flat"], groups[gi].t_flat,
-                                            mode=mred.MEDIAN, ws=mws)
-            if ev_m is not None:
-                ev_m[gi][1].record()
-            mred.reduce(plans[gi], d["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode,
-                        events=None if ev_s is None else ev_s[gi])
+            if st is not None:
+                st.wait_event(fork)
+            with torch.cuda.stream(st) if st is not None else contextlib.nullcontext():
+                if ev_m is not None:
+                    ev_m[gi][0].record()
+                MB, MD, MF = mred.build_masters(g, d["bias"], d["dark"], groups[gi].t_dark, d["flat"], groups[gi].t_flat,
+                                                mode=mred.MEDIAN, ws=mwss[gi % len(streams)], out=masters_out[gi])
+                masters_out[gi] = (MB, MD, MF)
+                if ev_m is not None:
+                    ev_m[gi][1].record()
+                mred.reduce(plans[gi], d["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode,
+                            events=None if ev_s is None else ev_s[gi])
+        for st in streams:
+            if st is not None:
+                join = torch.cuda.Event()
+                join.record(st)
+                main.wait_event(join)
 
     def new_events():
         E = lambda: torch.cuda.Event(enable_timing=True)
@@ -274,6 +304,24 @@ def run_ours(args):
             st_ms["build_masters"].append(evm[gi][0].elapsed_time(evm[gi][1]))
             for i, nmst in enumerate(STAGES):
                 st_ms[nmst].append(evs[gi][i].elapsed_time(evs[gi][i + 1]))
+    # the same step once more with every group on ONE stream: per-stage durations without overlap between groups
+    iso_ms = None
+    if len(streams) > 1:
+        keep, streams[:] = list(streams), [None]
+        iso_ev = []
+        for _ in range(max(3, args.steps)):
+            flush.fill_(1)
+            evm, evs = new_events()
+            step(evm, evs)
+            iso_ev.append((evm, evs))
+        barrier()
+        streams[:] = keep
+        iso_ms = {k: [] for k in ["build_masters"] + STAGES}
+        for evm, evs in iso_ev:
+            for gi in range(G):
+                iso_ms["build_masters"].append(evm[gi][0].elapsed_time(evm[gi][1]))
+                for i, nmst in enumerate(STAGES):
+                    iso_ms[nmst].append(evs[gi][i].elapsed_time(evs[gi][i + 1]))
     peaks = {}
     pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk_path):
@@ -285,6 +333,13 @@ def run_ours(args):
         gbs = sb[k] / (ms * 1e-3) / 1e9
         stages[k] = {"ms_per_call": round(ms, 5), "algorithmic_MB": round(sb[k] / 1e6, 3), "GBps": round(gbs, 1),
                      "frac": round(gbs / peak, 4)}
+    stages_iso = None
+    if iso_ms is not None:
+        stages_iso = {}
+        for k, v in iso_ms.items():
+            ms = float(np.mean(v))
+            gbs = sb[k] / (ms * 1e-3) / 1e9
+            stages_iso[k] = {"ms_per_call": round(ms, 5), "GBps": round(gbs, 1), "frac": round(gbs / peak, 4)}
     dom = max(STAGES, key=lambda k: np.sum(st_ms[k]))
     kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_finalize, k_correlate)",
             "resample": "k_resample", "coadd": "k_coadd"}[dom]
@@ -335,10 +390,16 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu:
         plan = oracle_sample_plan(cfg)
         grp = synth.make_group(cfg, 0, **plan)
-        s, nf, per = time_oracle_group(grp, lag)
+        s, nf, per, reps = 0.0, 0, {}, 0
+        while s < 10.0 and reps < 50:                      # ~10-30 s of single-thread CPU work
+            s1, n1, p1 = time_oracle_group(grp, lag)
+            s += s1
+            nf += n1
+            reps += 1
+            per = {k: per.get(k, 0.0) + v for k, v in p1.items()}
         cpu = {"value": nf / s, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": "1 group, %d science + %d/%d/%d masters (config %d shapes), %.1f s" % (
-                   plan["n_sci"], plan["n_master"], plan["n_master"], plan["n_master"], cfg, s),
+               "sample": "%d x (1 group, %d science + %d/%d/%d masters, config %d shapes), %.1f s" % (
+                   reps, plan["n_sci"], plan["n_master"], plan["n_master"], plan["n_master"], cfg, s),
                "stage_seconds": {k: round(v, 3) for k, v in per.items()}, "host_cores_available": os.cpu_count()}
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -347,9 +408,9 @@ def run_ours(args):
                 "config": {"workload": workload_name(cfg), "frames_per_step_per_gpu": G * n,
                            "includes": "build_masters + calibrate + estimate_shifts + resample + coadd per group",
                            "coadd": ["median", "mean", "sigclip 3.0 x3"][mode], "l2": "512 MB flush before every step",
-                           "parallelism": "groups sharded over ranks, no collective"},
+                           "parallelism": "groups sharded over ranks, no collective", "streams": len(streams)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + KERNELS_PER_REDUCE),
-                "roofline": roof, "stages": stages, "path_roofline": e2e_roof, "cpu_baseline": cpu,
+                "roofline": roof, "stages": stages, "stages_isolated": stages_iso, "path_roofline": e2e_roof, "cpu_baseline": cpu,
                 "wall_s_timed_region": round(wall, 4), "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU "
                 "stages on a TITAN X (Pascal) = ~870 frames/s (other hardware, other data; context only)"}
         print(json.dumps(line), flush=True)

@@ -102,11 +102,12 @@ def _ws(ws, need, device):
     return ws
 
 
-def build_masters(g, bias, dark, t_dark, flat, t_flat, mode=MEDIAN, ksigma=3.0, max_iter=3, ws=None, stream=None):
+def build_masters(g, bias, dark, t_dark, flat, t_flat, mode=MEDIAN, ksigma=3.0, max_iter=3, ws=None, stream=None,
+                  out=None):
     """include/mred.h: mred_build_masters.  Returns (MB, MD, MF) float32 [h][w] CUDA tensors."""
     gg = geom(g)
     dev = bias.device
-    MB, MD, MF = (torch.empty((gg.h, gg.w), dtype=torch.float32, device=dev) for _ in range(3))
+    MB, MD, MF = out if out is not None else (torch.empty((gg.h, gg.w), dtype=torch.float32, device=dev) for _ in range(3))
     nmax = max(bias.shape[0], dark.shape[0], flat.shape[0])
     ws = _ws(ws, workspace_bytes(CALL_BUILD_MASTERS, gg, nmax), dev)
     o = _opts(mode, ksigma, max_iter)

@@ -13,7 +13,7 @@ namespace mred {
 // (used for <F_k> of the flats).  Integer atomics -> order-independent, bit-exact.
 // grid (row_chunks, n), block 256; each warp takes rows r0 + warp, r0 + warp + 8, ...
 // ---------------------------------------------------------------------------------------------
-constexpr int SUM_ROWS = 32;
+constexpr int SUM_ROWS = 8;     // one row per warp
 
 __global__ void __launch_bounds__(256) k_frame_sums(const uint16_t* __restrict__ raw, Geom g, int n,
                                                     unsigned long long* __restrict__ os_sum,

@@ -52,7 +52,7 @@ size_t masters_ws_bytes(const Geom& g, int n)
 
 // Exact integer sums of all three stacks in one launch: overscan columns of every frame, and the image
 // rectangle of the flats (for <F_k>).  grid (row_chunks, nb+nd+nf), block 256; integer atomics -> bit-exact.
-constexpr int MSUM_ROWS = 32;
+constexpr int MSUM_ROWS = 8;    // one row per warp: 128 x (nb+nd+nf) blocks keep the loads of a 20-MB pass in flight
 __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict__ bias, int nb,
                                                      const uint16_t* __restrict__ dark, int nd,
                                                      const uint16_t* __restrict__ flat, int nf, Geom g,
@@ -75,7 +75,16 @@ __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict_
             unsigned long long b = 0;
             if (pair_ok) {      // two pixels per 32-bit load
                 const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
-                for (int x = lane; x < (g.w >> 1); x += 32) { const unsigned int v = __ldg(row2 + x); b += (v & 0xffffu) + (v >> 16); }
+                const int w2 = g.w >> 1;
+                int x = lane;
+                for (; x + 7 * 32 < w2; x += 8 * 32) {     // 8 independent loads in flight
+                    unsigned int v[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) v[u] = __ldg(row2 + x + 32 * u);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) b += (v[u] & 0xffffu) + (v[u] >> 16);
+                }
+                for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); b += (v & 0xffffu) + (v >> 16); }
             } else {
                 for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
             }
