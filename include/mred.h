@@ -26,6 +26,7 @@
  *    16-byte aligned; its contents are undefined afterwards and it must not be shared by calls
  *    that may run concurrently.
  *  - Frame counts: 1 <= n <= MRED_MAX_STACK (255) for every per-pixel-column call.
+ *  - One plane (W x H raw, w x h image) must hold fewer than 2^31 pixels (MRED_EINVAL otherwise).
  */
 #ifndef MRED_H
 #define MRED_H

@@ -182,6 +182,7 @@ int mred_coadd(const float* stack, int n, int w, int h, const int32_t* footprint
                float* out, uint16_t* count, uint32_t* rejmask, void* stream)
 {
     if (!stack || !out || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1 || !opts_ok(opts)) return MRED_EINVAL;
+    if ((int64_t)w * h >= (int64_t)1 << 31) return MRED_EINVAL;
     if (!aligned16(stack) || !aligned16(out) || (count && !aligned16(count)) || (rejmask && !aligned16(rejmask)))
         return MRED_EALIGN;
     return launch_coadd(stack, n, w, h, footprint, nullptr, *opts, out, count, rejmask,

@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
     const int w4 = (g.w + 3) >> 2;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (long long)g.h * w4) return;
-    const int y = (int)(gid / w4), x = (int)(gid - (long long)y * w4) * 4;
+    const int y = (int)((unsigned)gid / (unsigned)w4), x = (int)((unsigned)gid - (unsigned)y * (unsigned)w4) * 4;   // w*h < 2^31 (api.cu)
     const int nv = min(4, g.w - x);
     const size_t p = (size_t)y * g.w + x;
     float mb[4], ms[4], inv[4];

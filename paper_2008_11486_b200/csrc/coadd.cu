@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
     {
         const size_t p0 = (size_t)blockIdx.x * blockDim.x;
         const size_t p1 = min(p0 + blockDim.x, np) - 1;
-        const int ya = (int)(p0 / w), yb = (int)(p1 / w);
+        const int ya = (int)((unsigned)p0 / (unsigned)w), yb = (int)((unsigned)p1 / (unsigned)w);   // w*h < 2^31 (api.cu)
         const int xa = (int)(p0 - (size_t)ya * w), xb = (int)(p1 - (size_t)yb * w);
         const int k = threadIdx.x;
         if (k < NW * 32) {
@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
     }
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
-    const int y = (int)(p / w), x = (int)(p - (size_t)y * w);
+    const int y = (int)((unsigned)p / (unsigned)w), x = (int)((unsigned)p - (unsigned)y * (unsigned)w);
     const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
     float v[NMAX];
     uint32_t inside[NW];

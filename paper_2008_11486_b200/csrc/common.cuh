@@ -23,6 +23,7 @@ inline bool geom_ok(const mred_geom* g)
     if (g->W < 1 || g->H < 1 || g->w < 1 || g->h < 1) return false;
     if (g->x0 < 0 || g->y0 < 0 || (int64_t)g->x0 + g->w > g->W || (int64_t)g->y0 + g->h > g->H) return false;
     if (g->os_x0 < 0 || g->os_x1 < g->os_x0 || g->os_x1 > g->W) return false;
+    if ((int64_t)g->W * g->H >= (int64_t)1 << 31) return false;   // kernels index one plane with 32 bits
     return true;
 }
 

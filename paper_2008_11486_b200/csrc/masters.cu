@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
 #pragma unroll
     for (int i = 0; i < PX; ++i) { mb[i] = 0.f; md[i] = 0.f; }
     if (gid < (long long)g.h * wg) {
-        const int y = (int)(gid / wg), x = (int)(gid - (long long)y * wg) * PX;
+        const int y = (int)((unsigned)gid / (unsigned)wg), x = (int)((unsigned)gid - (unsigned)y * (unsigned)wg) * PX;   // w*h < 2^31
         const int nv = min(PX, g.w - x);
         const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
         const size_t p = (size_t)y * g.w + x;
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
 #pragma unroll
     for (int i = 0; i < PX; ++i) mf[i] = 0.f;
     if (gid < (long long)g.h * wg) {
-        const int y = (int)(gid / wg), x = (int)(gid - (long long)y * wg) * PX;
+        const int y = (int)((unsigned)gid / (unsigned)wg), x = (int)((unsigned)gid - (unsigned)y * (unsigned)wg) * PX;
         const int nv = min(PX, g.w - x);
         const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
         const size_t p = (size_t)y * g.w + x;
