@@ -13,43 +13,25 @@ namespace mred {
 // (used for <F_k> of the flats).  Integer atomics -> order-independent, bit-exact.
 // grid (row_chunks, n), block 256; each warp takes rows r0 + warp, r0 + warp + 8, ...
 // ---------------------------------------------------------------------------------------------
-constexpr int SUM_ROWS = 8;     // one row per warp
-
+// grid (ceil(H/256), n), block 256: one thread per row of the overscan strip
 __global__ void __launch_bounds__(256) k_frame_sums(const uint16_t* __restrict__ raw, Geom g, int n,
-                                                    unsigned long long* __restrict__ os_sum,
-                                                    unsigned long long* __restrict__ img_sum)
+                                                    unsigned long long* __restrict__ os_sum)
 {
     const int k = blockIdx.y;
-    const int r0 = blockIdx.x * SUM_ROWS;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint16_t* f = raw + (size_t)k * g.W * g.H;
-    unsigned long long s_os = 0, s_img = 0;
-    for (int r = r0 + warp; r < min(r0 + SUM_ROWS, g.H); r += 8) {
-        const uint16_t* row = f + (size_t)r * g.W;
-        unsigned int a = 0;
-        for (int x = g.os_x0 + lane; x < g.os_x1; x += 32) a += __ldg(row + x);
-        s_os += a;
-        if (img_sum && r >= g.y0 && r < g.y0 + g.h) {
-            unsigned long long b = 0;
-            for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
-            s_img += b;
-        }
-    }
-    s_os = warp_sum(s_os);
-    if (lane == 0 && s_os) atomicAdd(os_sum + k, s_os);
-    if (img_sum) {
-        s_img = warp_sum(s_img);
-        if (lane == 0 && s_img) atomicAdd(img_sum + k, s_img);
-    }
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long s = 0;
+    if (r < g.H) s = overscan_row_sum(raw + (size_t)k * g.W * g.H, g.W, g.os_x0, g.os_x1, r);
+    s = warp_sum(s);
+    if ((threadIdx.x & 31) == 0 && s) atomicAdd(os_sum + k, s);
 }
 
 int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long long* os_sum,
-                      unsigned long long* img_sum, cudaStream_t st)
+                      unsigned long long* /*img_sum*/, cudaStream_t st)
 {
     MRED_CUDA_TRY(cudaMemsetAsync(os_sum, 0, sizeof(unsigned long long) * n, st));
-    if (img_sum) MRED_CUDA_TRY(cudaMemsetAsync(img_sum, 0, sizeof(unsigned long long) * n, st));
-    dim3 grid((g.H + SUM_ROWS - 1) / SUM_ROWS, n);
-    k_frame_sums<<<grid, 256, 0, st>>>(raw, g, n, os_sum, img_sum);
+    if (g.os_x1 <= g.os_x0) return MRED_OK;
+    dim3 grid((g.H + 255) / 256, n);
+    k_frame_sums<<<grid, 256, 0, st>>>(raw, g, n, os_sum);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }

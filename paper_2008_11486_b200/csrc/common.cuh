@@ -71,6 +71,22 @@ __device__ __forceinline__ int warp_sum(int v)
     return v;
 }
 
+// Sum of the overscan pixels of row r of frame f (one THREAD per row: its ~50 loads are independent, so a warp
+// keeps 32 rows x 4 sectors in flight; rows are 2W bytes apart, so lanes never share a sector anyway).
+__device__ __forceinline__ unsigned int overscan_row_sum(const uint16_t* __restrict__ f, int W, int os_x0, int os_x1, int r)
+{
+    const uint16_t* row = f + (size_t)r * W;
+    unsigned int a = 0;
+    int x = os_x0;
+    if (((reinterpret_cast<uintptr_t>(row + x)) & 3u) && x < os_x1) a += __ldg(row + x++);     // align to 4 bytes
+    const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + x);
+    const int n2 = (os_x1 - x) >> 1;
+#pragma unroll 8
+    for (int i = 0; i < n2; ++i) { const unsigned int v = __ldg(row2 + i); a += (v & 0xffffu) + (v >> 16); }
+    if (x + 2 * n2 < os_x1) a += __ldg(row + x + 2 * n2);
+    return a;
+}
+
 // footprint of a shift along one axis of length n: [max(0, ceil(s)), min(n-1, floor(n-1+s))]
 // (O5).  Same IEEE double operations on host and device.
 __host__ __device__ inline void axis_footprint(int n, double s, int& lo, int& hi)

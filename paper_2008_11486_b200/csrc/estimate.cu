@@ -4,15 +4,15 @@
 //
 //   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): float64 column
 //                partial sums per 64-row band and complete float64 row sums, valid-pixel counts.
-//   k_finalize : per (frame, axis): fixed-order band sum, mean, median by a shared-memory bitonic sort, subtract.
-//   k_correlate: per (frame, axis): C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
+//   k_shifts   : per (frame, axis): fixed-order band sum, mean, median by a shared-memory radix select, subtract
+//                (for the reference and for the frame), then C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
 //                smaller |l| then smaller l; 3-point parabola.
 // No float atomics: every sum has a fixed order, so the integer result is reproducible.
 #include "common.cuh"
 
 namespace mred {
 
-constexpr int PROF_BR = 16;        // rows per band
+constexpr int PROF_BR = 32;        // rows per band
 constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
 
 struct EstimateWs {
@@ -113,20 +113,71 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
     }
 }
 
-// grid (n, 2): axis 0 = x profile (length w), axis 1 = y profile (length h).  Mean profile, then its median
-// by a bitonic sort in shared memory (invalid lines sort to the end as +inf), then the subtraction.
-__global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
+// order-preserving map double -> uint64
+__device__ __forceinline__ unsigned long long key_of(double v)
 {
-    __shared__ double s_p[PROF_MAXLEN];
-    __shared__ int s_m;
-    const int k = blockIdx.x, axis = blockIdx.y;
-    const int len = axis == 0 ? w : h;
-    int P = 1;
-    while (P < len) P <<= 1;
-    if (threadIdx.x == 0) s_m = 0;
-    __syncthreads();
-    double* out = e.prof + ((size_t)k * 2 + axis) * e.plen;
+    const unsigned long long u = (unsigned long long)__double_as_longlong(v);
+    return (u >> 63) ? ~u : (u | 0x8000000000000000ULL);
+}
+__device__ __forceinline__ double val_of(unsigned long long k)
+{
+    const unsigned long long u = (k >> 63) ? (k & 0x7fffffffffffffffULL) : ~k;
+    return __longlong_as_double((long long)u);
+}
+
+struct SelectScratch { unsigned int hist[256]; unsigned long long prefix; unsigned int rank; unsigned long long red[32]; };
+
+// key of rank r (0-based, ascending) among keys[0..P): 8-bit radix select, 8 passes (block-wide call)
+__device__ unsigned long long block_select(const unsigned long long* keys, int P, unsigned int r, SelectScratch* sc)
+{
+    if (threadIdx.x == 0) { sc->prefix = 0ULL; sc->rank = r; }
+    unsigned long long mask = 0ULL;
+    for (int shift = 56; shift >= 0; shift -= 8) {
+        for (int i = threadIdx.x; i < 256; i += blockDim.x) sc->hist[i] = 0u;
+        __syncthreads();
+        const unsigned long long prefix = sc->prefix;
+        for (int i = threadIdx.x; i < P; i += blockDim.x) {
+            // profile values share their leading bytes, so a pass would send a whole warp to one bin:
+            // aggregate equal digits inside the warp first (one shared-memory atomic per distinct digit)
+            const unsigned long long k = keys[i];
+            const unsigned int am = __activemask();
+            const unsigned int d = ((k & mask) == prefix) ? ((unsigned int)(k >> shift) & 255u) : 256u;
+            const unsigned int same = __match_any_sync(am, d);
+            if (d < 256u && (threadIdx.x & 31) == (unsigned int)(__ffs(same) - 1)) atomicAdd(&sc->hist[d], (unsigned int)__popc(same));
+        }
+        __syncthreads();
+        if (threadIdx.x < 32) {          // warp 0: find the bin that holds the rank (8 bins per lane)
+            const int lane = threadIdx.x;
+            unsigned int loc[8], tot = 0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { loc[u] = sc->hist[8 * lane + u]; tot += loc[u]; }
+            unsigned int inc = tot;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+            const unsigned int before = inc - tot, rk = sc->rank;
+            if (rk >= before && rk < inc) {          // exactly one lane
+                unsigned int cum = before;
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    if (rk >= cum && rk < cum + loc[u]) { sc->prefix = prefix | ((unsigned long long)(8 * lane + u) << shift); sc->rank = rk - cum; }
+                    cum += loc[u];
+                }
+            }
+        }
+        mask |= 255ULL << shift;
+        __syncthreads();
+    }
+    return sc->prefix;
+}
+
+// Median-subtracted mean profile of frame k along `axis` into dst[0..len) (shared memory); keys[0..P) is scratch
+// for the selection (invalid lines get the +inf key, which sorts last).  All threads of the block call it.
+__device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis, int len, int P, double* dst,
+                              unsigned long long* keys, SelectScratch* sc, int* s_m)
+{
     const double INF = __longlong_as_double(0x7ff0000000000000LL);
+    if (threadIdx.x == 0) *s_m = 0;
+    __syncthreads();
     int mine = 0;
     for (int i = threadIdx.x; i < P; i += blockDim.x) {
         double v = INF;
@@ -134,59 +185,90 @@ __global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
             double s = 0.0;
             int c = 0;
             if (axis == 0) {
-                for (int b = 0; b < e.nbands; ++b) {
-                    s += e.colpart[((size_t)k * e.nbands + b) * w + i];
-                    c += e.colcnt[((size_t)k * e.nbands + b) * w + i];
+                const double* cp = e.colpart + (size_t)k * e.nbands * w + i;
+                const int* cc = e.colcnt + (size_t)k * e.nbands * w + i;
+                int b = 0;
+                for (; b + 8 <= e.nbands; b += 8) {          // 8 bands in flight; the order of the adds stays fixed
+                    double tv[8];
+                    int tc[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) { tv[u] = __ldcg(cp + (size_t)(b + u) * w); tc[u] = __ldcg(cc + (size_t)(b + u) * w); }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) { s += tv[u]; c += tc[u]; }
                 }
+                for (; b < e.nbands; ++b) { s += __ldcg(cp + (size_t)b * w); c += __ldcg(cc + (size_t)b * w); }
             } else {
-                s = e.rowsum[(size_t)k * h + i];
-                c = e.rowcnt[(size_t)k * h + i];
+                s = __ldcg(e.rowsum + (size_t)k * h + i);
+                c = __ldcg(e.rowcnt + (size_t)k * h + i);
             }
             if (c > 0) { v = s / (double)c; ++mine; }
-            out[i] = v;
+            dst[i] = v;
         }
-        s_p[i] = v;
+        keys[i] = key_of(v);
     }
-    if (mine) atomicAdd(&s_m, mine);
+    if (mine) atomicAdd(s_m, mine);
     __syncthreads();
-    for (int kk = 2; kk <= P; kk <<= 1) {
-        for (int j = kk >> 1; j > 0; j >>= 1) {
+    const int m = *s_m;
+    double med = 0.0;
+    if (m > 0) {
+        const unsigned long long ka = block_select(keys, P, (unsigned int)((m - 1) >> 1), sc);
+        med = val_of(ka);
+        if (!(m & 1)) {
+            // rank m/2 = next order statistic: ka again if it is repeated often enough, else the smallest key above it
+            unsigned int le = 0;
+            unsigned long long mn = ~0ULL;
             for (int i = threadIdx.x; i < P; i += blockDim.x) {
-                const int l = i ^ j;
-                if (l > i) {
-                    const double a = s_p[i], b = s_p[l];
-                    const bool up = (i & kk) == 0;
-                    if ((a > b) == up) { s_p[i] = b; s_p[l] = a; }
-                }
+                const unsigned long long kk = keys[i];
+                le += kk <= ka;
+                if (kk > ka && kk < mn) mn = kk;
             }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                le += __shfl_xor_sync(0xffffffffu, le, o);
+                const unsigned long long t = __shfl_xor_sync(0xffffffffu, mn, o);
+                mn = t < mn ? t : mn;
+            }
+            __syncthreads();
+            if ((threadIdx.x & 31) == 0) { sc->red[threadIdx.x >> 5] = mn; sc->hist[threadIdx.x >> 5] = le; }
+            __syncthreads();
+            unsigned int le_all = 0;
+            unsigned long long mn_all = ~0ULL;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { le_all += sc->hist[i]; mn_all = sc->red[i] < mn_all ? sc->red[i] : mn_all; }
+            const double b = (le_all > (unsigned int)(m >> 1)) ? med : val_of(mn_all);
+            med = 0.5 * (med + b);
             __syncthreads();
         }
     }
-    const int m = s_m;
-    double med = 0.0;
-    if (m > 0) {
-        const double a = s_p[(m - 1) >> 1], b = s_p[m >> 1];
-        med = (m & 1) ? a : 0.5 * (a + b);
-    }
     for (int i = threadIdx.x; i < len; i += blockDim.x) {
-        const double v = out[i];
-        out[i] = (v == INF) ? 0.0 : v - med;
+        const double v = dst[i];
+        dst[i] = (v == INF) ? 0.0 : v - med;
     }
+    __syncthreads();
 }
 
-// grid (n, 2), block 1024: one lag per warp and round
-__global__ void __launch_bounds__(1024) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
-                                                   int32_t* __restrict__ ishift, double* __restrict__ shift)
+// grid (n, 2), block 1024: block (k, axis) builds the reference profile and its own (each block redoes the
+// reference: 2n tiny blocks run in parallel, and no block waits for another), then the 2R+1 lags, one per warp
+// and round, from shared memory; argmax with ties to the smaller |l| then smaller l; 3-point parabola.
+__global__ void __launch_bounds__(1024) k_shifts(int w, int h, int n, int ref, int R, EstimateWs e,
+                                                 int32_t* __restrict__ ishift, double* __restrict__ shift)
 {
+    extern __shared__ double s_dyn[];     // a[P], b[P], selection keys[P]
     __shared__ double s_C[2 * MRED_MAX_LAG + 1];
+    __shared__ SelectScratch s_sc;
+    __shared__ int s_m;
     const int k = blockIdx.x, axis = blockIdx.y;
     if (k == ref) {
         if (threadIdx.x == 0) { ishift[2 * k + axis] = 0; shift[2 * k + axis] = 0.0; }
         return;
     }
     const int len = axis == 0 ? w : h;
-    const double* a = e.prof + ((size_t)ref * 2 + axis) * e.plen;
-    const double* b = e.prof + ((size_t)k * 2 + axis) * e.plen;
+    int P = 1;
+    while (P < len) P <<= 1;
+    double* a = s_dyn;
+    double* b = s_dyn + P;
+    unsigned long long* keys = reinterpret_cast<unsigned long long*>(s_dyn + 2 * P);
+    block_profile(e, w, h, ref, axis, len, P, a, keys, &s_sc, &s_m);
+    block_profile(e, w, h, k, axis, len, P, b, keys, &s_sc, &s_m);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int l = -R + warp; l <= R; l += 32) {
         const int j0 = max(0, -l), j1 = min(len, len - l);
@@ -225,9 +307,15 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     const int vec_ok = (w % 4 == 0) ? 1 : 0;
     k_profiles<<<dim3(e.nbands, n), 256, 0, st>>>(frames, w, h, bad, e, vec_ok);
     MRED_LAUNCH_CHECK();
-    k_finalize<<<dim3(n, 2), 1024, 0, st>>>(w, h, e);
-    MRED_LAUNCH_CHECK();
-    k_correlate<<<dim3(n, 2), 1024, 0, st>>>(w, h, n, ref, max_lag, e, ishift, shift);
+    int P = 1;
+    while (P < (w > h ? w : h)) P <<= 1;
+    const size_t smem = 3 * (size_t)P * sizeof(double);
+    static bool attr_done = false;   // idempotent
+    if (!attr_done) {
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_shifts, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * PROF_MAXLEN * (int)sizeof(double)));
+        attr_done = true;
+    }
+    k_shifts<<<dim3(n, 2), 1024, smem, st>>>(w, h, n, ref, max_lag, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }

@@ -50,53 +50,49 @@ size_t masters_ws_bytes(const Geom& g, int n)
     return carve(nullptr, g, n, n, n).bytes;   // n = max(nb, nd, nf) is an upper bound for each
 }
 
-// Exact integer sums of all three stacks in one launch: overscan columns of every frame, and the image
-// rectangle of the flats (for <F_k>).  grid (row_chunks, nb+nd+nf), block 256; integer atomics -> bit-exact.
-constexpr int MSUM_ROWS = 8;    // one row per warp: 128 x (nb+nd+nf) blocks keep the loads of a 20-MB pass in flight
+// Exact integer sums of all three stacks in one launch: overscan columns of every frame (blocks
+// x < nos: one thread per row), and the image rectangle of the flats for <F_k> (blocks x >= nos: one row per
+// warp, coalesced).  grid (nos + nimg, nb+nd+nf), block 256; integer atomics -> bit-exact.
 __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict__ bias, int nb,
                                                      const uint16_t* __restrict__ dark, int nd,
-                                                     const uint16_t* __restrict__ flat, int nf, Geom g,
+                                                     const uint16_t* __restrict__ flat, int nf, Geom g, int nos,
                                                      unsigned long long* __restrict__ os,
                                                      unsigned long long* __restrict__ img_f, int pair_ok)
 {
     const int k = blockIdx.y;
     const size_t fs = (size_t)g.W * g.H;
     const uint16_t* f = k < nb ? bias + (size_t)k * fs : (k < nb + nd ? dark + (size_t)(k - nb) * fs : flat + (size_t)(k - nb - nd) * fs);
-    const bool want_img = k >= nb + nd;
-    const int r0 = blockIdx.x * MSUM_ROWS;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    unsigned long long s_os = 0, s_img = 0;
-    for (int r = r0 + warp; r < min(r0 + MSUM_ROWS, g.H); r += 8) {
-        const uint16_t* row = f + (size_t)r * g.W;
-        unsigned int a = 0;
-        for (int x = g.os_x0 + lane; x < g.os_x1; x += 32) a += __ldg(row + x);
-        s_os += a;
-        if (want_img && r >= g.y0 && r < g.y0 + g.h) {
-            unsigned long long b = 0;
-            if (pair_ok) {      // two pixels per 32-bit load
-                const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
-                const int w2 = g.w >> 1;
-                int x = lane;
-                for (; x + 7 * 32 < w2; x += 8 * 32) {     // 8 independent loads in flight
-                    unsigned int v[8];
+    if ((int)blockIdx.x < nos) {
+        const int r = blockIdx.x * blockDim.x + threadIdx.x;
+        unsigned long long s = 0;
+        if (r < g.H && g.os_x1 > g.os_x0) s = overscan_row_sum(f, g.W, g.os_x0, g.os_x1, r);
+        s = warp_sum(s);
+        if (lane == 0 && s) atomicAdd(os + k, s);
+        return;
+    }
+    if (k < nb + nd) return;                       // image sums: flats only
+    const int r = g.y0 + ((int)blockIdx.x - nos) * 8 + warp;
+    if (r >= g.y0 + g.h) return;
+    const uint16_t* row = f + (size_t)r * g.W;
+    unsigned long long b = 0;
+    if (pair_ok) {      // two pixels per 32-bit load, 8 independent loads in flight
+        const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
+        const int w2 = g.w >> 1;
+        int x = lane;
+        for (; x + 7 * 32 < w2; x += 8 * 32) {
+            unsigned int v[8];
 #pragma unroll
-                    for (int u = 0; u < 8; ++u) v[u] = __ldg(row2 + x + 32 * u);
+            for (int u = 0; u < 8; ++u) v[u] = __ldg(row2 + x + 32 * u);
 #pragma unroll
-                    for (int u = 0; u < 8; ++u) b += (v[u] & 0xffffu) + (v[u] >> 16);
-                }
-                for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); b += (v & 0xffffu) + (v >> 16); }
-            } else {
-                for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
-            }
-            s_img += b;
+            for (int u = 0; u < 8; ++u) b += (v[u] & 0xffffu) + (v[u] >> 16);
         }
+        for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); b += (v & 0xffffu) + (v >> 16); }
+    } else {
+        for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
     }
-    s_os = warp_sum(s_os);
-    if (lane == 0 && s_os) atomicAdd(os + k, s_os);
-    if (want_img) {
-        s_img = warp_sum(s_img);
-        if (lane == 0 && s_img) atomicAdd(img_f + (k - nb - nd), s_img);
-    }
+    b = warp_sum(b);
+    if (lane == 0 && b) atomicAdd(img_f + (k - nb - nd), b);
 }
 
 // deterministic block sum of one double per thread (256 threads): shuffle tree, then warp 0 adds the
@@ -348,8 +344,8 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     MRED_CUDA_TRY(cudaMemsetAsync(m.os, 0, m.zero_bytes, st));
     // pairs of pixels by one 32-bit load need even W, x0 and w (frame bases are 16-byte aligned, frames W*H*2 B)
     const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0 && g.w % 2 == 0 && ((size_t)g.W * g.H) % 2 == 0) ? 1 : 0;
-    k_master_sums<<<dim3((g.H + MSUM_ROWS - 1) / MSUM_ROWS, nb + nd + nf), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, m.os,
-                                                                                     m.img_f, pair_ok);
+    const int nos = (g.H + 255) / 256, nimg = (g.h + 7) / 8;
+    k_master_sums<<<dim3(nos + nimg, nb + nd + nf), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, nos, m.os, m.img_f, pair_ok);
     MRED_LAUNCH_CHECK();
     const size_t np = (size_t)g.w * g.h;
     const int nbd = nb > nd ? nb : nd;
