@@ -51,12 +51,28 @@ def workload_name(cfg):
         cfg, sp["groups"], sp["n_sci"], sp["n_master"], sp["n_master"], sp["n_master"], g.W, g.H)
 
 
+def rank_group_ids(cfg, rank):
+    """Group numbers (= seed offsets) this rank reduces.  Weak scaling: every rank gets its own full copy of the
+    config, seeded apart; groups are independent, so there is no data-path collective."""
+    return [gi + 100 * rank for gi in range(synth.CONFIGS[cfg]["groups"])]
+
+
 def make_groups(cfg, rank):
-    """All groups of the config for this rank (weak scaling: every rank gets its own full copy, seeded apart)."""
-    sp = synth.CONFIGS[cfg]
     from concurrent.futures import ThreadPoolExecutor
-    with ThreadPoolExecutor(max_workers=min(8, sp["groups"])) as ex:
-        return list(ex.map(lambda gi: synth.make_group(cfg, gi + 100 * rank), range(sp["groups"])))
+    ids = rank_group_ids(cfg, rank)
+    with ThreadPoolExecutor(max_workers=min(8, len(ids))) as ex:
+        return list(ex.map(lambda gid: synth.make_group(cfg, gid), ids))
+
+
+def max_over_ranks(value, device=None):
+    """Max of a per-rank scalar over the process group (the only collective bench.py issues); identity without one."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def stage_bytes(g, n, nm, want_mask_words=0):
@@ -188,8 +204,8 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------
-KERNELS_PER_BUILD_MASTERS = 8    # 3 x k_frame_sums, k_masters_bd, k_flat_means, k_masters_f, k_mf_mean, k_mf_scale
-KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd
+KERNELS_PER_BUILD_MASTERS = 4    # k_master_sums, k_masters_bd, k_masters_f, k_mf_scale
+KERNELS_PER_REDUCE = 6           # k_frame_sums, k_calibrate, k_profiles, k_shifts, k_resample, k_coadd
 
 
 def run_ours(args):
@@ -316,10 +332,7 @@ def run_ours(args):
         barrier()
     step_ms = [a.elapsed_time(b) for a, b in step_ev]
     total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=devs)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, devs)
     frames_per_step = G * n * world
     value = frames_per_step * args.steps / (total_ms * 1e-3)
 
@@ -368,10 +381,14 @@ def run_ours(args):
             gbs = sb[k] / (ms * 1e-3) / 1e9
             stages_iso[k] = {"ms_per_call": round(ms, 5), "GBps": round(gbs, 1), "frac": round(gbs / peak, 4)}
     dom = max(STAGES, key=lambda k: np.sum(st_ms[k]))
-    kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_finalize, k_correlate)",
+    kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_shifts)",
             "resample": "k_resample", "coadd": "k_coadd"}[dom]
+    traffic = None
+    tr_path = os.path.join(ROOT, "profiles", "traffic.json")      # ncu --set full capture of config 2 (profiles/r1f_kernels.md)
+    if cfg == 2 and os.path.exists(tr_path):
+        traffic = json.load(open(tr_path)).get(dom)
     roof = {"bound": "hbm", "kernel": kern, "stage": dom, "achieved": stages[dom]["GBps"], "peak": peak,
-            "peak_source": peak_src, "unit": "GB/s", "frac": stages[dom]["frac"], "traffic": None,
+            "peak_source": peak_src, "unit": "GB/s", "frac": stages[dom]["frac"], "traffic": traffic,
             "algorithmic_bytes_per_launch": sb[dom], "launch_ms": stages[dom]["ms_per_call"]}
     sci_bytes = sum(sb[k] for k in STAGES)
     sci_ms = sum(stages[k]["ms_per_call"] for k in STAGES)
@@ -403,10 +420,7 @@ def run_ours(args):
         b.record()
         barrier()
         ems = a.elapsed_time(b)
-        if world > 1:
-            t = torch.tensor([ems], dtype=torch.float64, device=devs)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
+        ems = max_over_ranks(ems, devs)
         raw = 2 * g.W * g.H
         e2e = {"value": frames_per_step * ks / (ems * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": G * (n + 3 * nm) * raw,
