@@ -156,9 +156,13 @@ def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stre
     return ish, sh
 
 
-def resample(frames, sx, sy, fill=0.0, out=None, stream=None):
-    """include/mred.h: mred_resample.  sx, sy: host float64 [n].  Returns (out, footprint int32 [n][4] numpy)."""
+def resample(frames, sx, sy, fill=0.0, out=None, ws=None, stream=None):
+    """include/mred.h: mred_resample.  sx, sy: host float64 [n].  Returns (out, footprint int32 [n][4] numpy).
+    ws: optional scratch of workspace_bytes(CALL_RESAMPLE, ...) bytes (allocated here when None and non-zero)."""
     n, h, w = frames.shape
+    need = workspace_bytes(CALL_RESAMPLE, Geom(0, 0, 0, 0, 0, 0, w, h), n)
+    if ws is None and need:
+        ws = torch.empty(need, dtype=torch.uint8, device=frames.device)
     sx = np.ascontiguousarray(np.broadcast_to(np.asarray(sx, np.float64), (n,)))
     sy = np.ascontiguousarray(np.broadcast_to(np.asarray(sy, np.float64), (n,)))
     if out is None:
@@ -166,8 +170,9 @@ def resample(frames, sx, sy, fill=0.0, out=None, stream=None):
     fp = np.zeros((n, 4), np.int32)
     rc = lib().mred_resample(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
                              sx.ctypes.data_as(C.c_void_p), sy.ctypes.data_as(C.c_void_p), C.c_float(fill),
-                             _dev(out, torch.float32, "out"), fp.ctypes.data_as(C.c_void_p), C.c_void_p(None),
-                             C.c_size_t(0), _stream(stream))
+                             _dev(out, torch.float32, "out"), fp.ctypes.data_as(C.c_void_p),
+                             C.c_void_p(ws.data_ptr() if ws is not None else None),
+                             C.c_size_t(ws.numel() if ws is not None else 0), _stream(stream))
     _check(rc, "mred_resample")
     return out, fp
 

@@ -26,6 +26,8 @@ struct ReduceWs {
     double* shift;            // [n][2]
     int32_t* fp;              // [n][4]
     void* est;                // estimate workspace
+    void* rs;                 // resample workspace (x-shifted stack, small stacks only)
+    size_t rs_bytes;
     size_t bytes;
 };
 
@@ -42,6 +44,8 @@ static ReduceWs carve_reduce(void* ws, const Geom& g, int n)
     r.shift = reinterpret_cast<double*>(take(16 * (size_t)n));
     r.fp = reinterpret_cast<int32_t*>(take(16 * (size_t)n));
     r.est = take(estimate_ws_bytes(g.w, g.h, n));
+    r.rs_bytes = resample_ws_bytes(g.w, g.h, n);
+    r.rs = take(r.rs_bytes);
     r.bytes = (size_t)(p - static_cast<char*>(ws));
     return r;
 }
@@ -99,7 +103,7 @@ size_t mred_workspace_bytes(int call, const mred_geom* geom, int n)
         case MRED_CALL_BUILD_MASTERS: return masters_ws_bytes(g, n);
         case MRED_CALL_CALIBRATE: return align_up(8 * (size_t)n, 16);
         case MRED_CALL_ESTIMATE_SHIFTS: return estimate_ws_bytes(g.w, g.h, n);
-        case MRED_CALL_RESAMPLE: return 0;
+        case MRED_CALL_RESAMPLE: return resample_ws_bytes(g.w, g.h, n);   /* optional: without it the one-kernel route runs */
         case MRED_CALL_COADD: return 0;
         case MRED_CALL_REDUCE: return carve_reduce(nullptr, g, n).bytes;
         default: return 0;
@@ -162,7 +166,7 @@ int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index
 int mred_resample(const float* in, int n, int w, int h, const double* sx, const double* sy, float fill,
                   float* out, int32_t* footprint, void* ws, size_t ws_bytes, void* stream)
 {
-    (void)ws; (void)ws_bytes;
+    if (ws && !aligned16(ws)) return MRED_EALIGN;
     if (!in || !out || !sx || !sy || n < 1 || n > MRED_MAX_STACK || w < 4 || h < 4 || in == out) return MRED_EINVAL;
     for (int k = 0; k < n; ++k)
         if (!isfinite(sx[k]) || !isfinite(sy[k]) || fabs(sx[k]) > 1.0e6 || fabs(sy[k]) > 1.0e6) return MRED_EINVAL;
@@ -175,7 +179,7 @@ int mred_resample(const float* in, int n, int w, int h, const double* sx, const 
             axis_footprint(h, sy[k], lo, hi);
             footprint[4 * k + 2] = lo; footprint[4 * k + 3] = hi;
         }
-    return launch_resample(in, n, w, h, sx, sy, nullptr, fill, out, nullptr, static_cast<cudaStream_t>(stream));
+    return launch_resample(in, n, w, h, sx, sy, nullptr, fill, out, nullptr, ws, ws_bytes, static_cast<cudaStream_t>(stream));
 }
 
 int mred_coadd(const float* stack, int n, int w, int h, const int32_t* footprint, const mred_comb_opts* opts,
@@ -217,7 +221,7 @@ int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float 
     int32_t* fp = footprint_out ? footprint_out : r.fp;
     if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, st))) return rc;
     MRED_STAGE_EVENT(2);
-    if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, st))) return rc;
+    if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, r.rs, r.rs_bytes, st))) return rc;
     MRED_STAGE_EVENT(3);
     if ((rc = launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st))) return rc;
     MRED_STAGE_EVENT(4);

@@ -114,6 +114,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
 size_t estimate_ws_bytes(int w, int h, int n);
 int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,
                     const double* dshift_dev /* [n][2] (dx,dy): shift = -d */, float fill, float* out,
-                    int32_t* fp_dev /* nullable */, cudaStream_t st);
+                    int32_t* fp_dev /* nullable */, void* ws /* nullable */, size_t ws_bytes, cudaStream_t st);
+size_t resample_ws_bytes(int w, int h, int n);
 
 }  // namespace mred

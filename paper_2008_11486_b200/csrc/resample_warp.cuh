@@ -306,16 +306,26 @@ __device__ __forceinline__ void sweep_block(const Item& it, const YCtx& yc, cons
     for (int j = 0; j < V; ++j) { s1[j] = cA[j]; s2[j] = n2[j]; s3[j] = n3[j]; }
 }
 
-template <bool VEC>
+// MODE 0: x and y pass fused (one read, one write per pixel).
+// MODE 1: x pass only, `out` = the x-shifted rows (every row of the band, no y footprint, no fill).
+// MODE 2: y pass only on x-shifted rows: no halo lanes, no realignment, columns map one to one.
+// Modes 1 + 2 are the two-kernel route for stacks small enough to keep the intermediate in L2.
+template <int MODE> struct ModeGeom {
+    static constexpr int HL = MODE == 2 ? 0 : HALO_L, HR = MODE == 2 ? 0 : HALO_R;
+    static constexpr int OUTC = (32 - HL - HR) * V;
+};
+
+template <bool VEC, int MODE>
 __device__ void warp_item(const Item& it, float* ring, int lane)
 {
+    constexpr int HL = ModeGeom<MODE>::HL, HR = ModeGeom<MODE>::HR, OUTC = ModeGeom<MODE>::OUTC;
     const Axis& ax = it.ax;
     const Axis& ay = it.ay;
     YCtx yc;
     yc.x0 = it.XA + V * lane;
-    yc.lane_on = lane >= HALO_L && lane < 32 - HALO_R && yc.x0 < it.w;
-    const int Xs = it.XA + V * HALO_L;                                 // first kept column of the strip
-    const int Xe = min(Xs + OUTCOLS, it.w);                            // one past the last
+    yc.lane_on = lane >= HL && lane < 32 - HR && yc.x0 < it.w;
+    const int Xs = it.XA + V * HL;                                     // first kept column of the strip
+    const int Xe = min(Xs + OUTC, it.w);                               // one past the last
     float fillv[V];
 #pragma unroll
     for (int j = 0; j < V; ++j) fillv[j] = it.fill;
@@ -323,12 +333,17 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
     // rows of the band that can hold data; everything else is fill
     const bool x_any = max(Xs, ax.lo) <= min(Xe - 1, ax.hi);
     int ylo = max(it.ya, ay.lo), yhi = min(it.yb - 1, ay.hi);
-    if (!x_any) { ylo = it.yb; yhi = it.yb - 1; }
-    for (int y = it.ya; y < min(ylo, it.yb); ++y) store_row<VEC>(it, y, yc.x0, yc.lane_on, fillv);
-    for (int y = max(yhi + 1, it.ya); y < it.yb; ++y) store_row<VEC>(it, y, yc.x0, yc.lane_on, fillv);
-    if (ylo > yhi) return;
+    if (MODE == 1) {
+        if (!x_any) return;                        // the y pass writes fill there without reading
+        ylo = it.ya; yhi = it.yb - 1;
+    } else {
+        if (!x_any) { ylo = it.yb; yhi = it.yb - 1; }
+        for (int y = it.ya; y < min(ylo, it.yb); ++y) store_row<VEC>(it, y, yc.x0, yc.lane_on, fillv);
+        for (int y = max(yhi + 1, it.ya); y < it.yb; ++y) store_row<VEC>(it, y, yc.x0, yc.lane_on, fillv);
+        if (ylo > yhi) return;
+    }
 
-    if (ax.ident && ay.ident) {     // pure integer translation: copy with 16 independent loads in flight per lane
+    if (MODE == 0 && ax.ident && ay.ident) {     // pure integer translation: copy with 16 independent loads in flight per lane
         const int xa = max(Xs, ax.lo), xb = min(Xe - 1, ax.hi);       // columns that carry data (x_any: xa <= xb)
         for (int y = ylo; y <= yhi; ++y) {                            // fill left and right of the footprint
             float* dst = it.out + (size_t)y * it.w;
@@ -397,11 +412,15 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
         if (yc.x0 + j >= ax.lo && yc.x0 + j <= ax.hi) yc.xmask |= 1u << j;
 
     // x geometry of the lane
-    const int KC0 = it.XA + ax.m;                 // source column under output column XA
-    const int r = VEC ? (KC0 & 3) : 0;            // aligned loads start r columns early
+    const int KC0 = MODE == 2 ? it.XA : it.XA + ax.m;   // source column under output column XA
+    const int r = (VEC && MODE != 2) ? (KC0 & 3) : 0;   // aligned loads start r columns early
     const int col_load = KC0 - r + V * lane;
     const bool simple = it.w >= 2 * EXT + 8 && it.h >= 2 * EXT + 8;
-    const HalfCfg h0 = half_cfg(col_load, it.w, VEC, simple), h1 = half_cfg(col_load + 4, it.w, VEC, simple);
+    HalfCfg h0 = half_cfg(col_load, it.w, VEC, simple), h1 = half_cfg(col_load + 4, it.w, VEC, simple);
+    if (MODE == 2) {                              // columns beyond the image are never stored: no reflection
+        if (h0.mode == 1) h0.mode = 4;
+        if (h1.mode == 1) h1.mode = 4;
+    }
     XFix xf;
     xf.l0 = h0.mode == 1 && h0.c < 0; xf.l1 = h1.mode == 1 && h1.c < 0;
     xf.r0 = h0.mode == 1 && h0.c > 0; xf.r1 = h1.mode == 1 && h1.c > 0;
@@ -417,8 +436,8 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
 
     // y schedule
     const int ka = ylo + ay.m, kb = yhi + 1 + ay.m;     // intervals [ka, kb)
-    const int r0 = ka - WARM;                           // first source row processed
-    const int NB = (kb - ka + 18) / RB + 3;             // blocks processed
+    const int r0 = MODE == 1 ? ylo : ka - WARM;         // first source row processed
+    const int NB = MODE == 1 ? (yhi - ylo + RB) / RB : (kb - ka + 18) / RB + 3;   // blocks (of RB rows) processed
 
     float gprev[V], A1[V], A2[V], s1[V], s2[V], s3[V];
 #pragma unroll
@@ -465,7 +484,7 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
 #pragma unroll
                 for (int i = 0; i < GR; ++i) x_fix(xf, cur[i]);
             }
-            if (row0 < 0 || row0 + GR > it.h) {
+            if (MODE != 1 && (row0 < 0 || row0 + GR > it.h)) {
 #pragma unroll 1
                 for (int i = 0; i < GR; ++i) {
                     const int row = row0 + i;
@@ -485,11 +504,19 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
                 }
             }
         }
-        if (VEC) {
+        if (MODE != 2) {
+            if (VEC) {
 #pragma unroll
-            for (int i = 0; i < GR; ++i) realign(cur[i], r);
+                for (int i = 0; i < GR; ++i) realign(cur[i], r);
+            }
+            x_pass<GR>(nax, nax8, wx, cur);
         }
-        x_pass<GR>(nax, nax8, wx, cur);
+        if (MODE == 1) {
+#pragma unroll
+            for (int i = 0; i < GR; ++i)
+                if (row0 + i <= yhi) store_row<VEC>(it, row0 + i, yc.x0, yc.lane_on, cur[i]);
+            continue;
+        }
 #pragma unroll
         for (int i = 0; i < GR; ++i) {
 #pragma unroll
@@ -522,7 +549,8 @@ __device__ void warp_item(const Item& it, float* ring, int lane)
 
 using namespace rs;
 
-__global__ void __launch_bounds__(32, 8) k_resample(const float* __restrict__ in, int n, int w, int h,
+template <int MODE>
+__global__ void __launch_bounds__(32, MODE == 1 ? 16 : 8) k_resample(const float* __restrict__ in, int n, int w, int h,
                                                      const __grid_constant__ HostShifts hs,
                                                      const double* __restrict__ dshift, float fill,
                                                      float* __restrict__ out, int4* __restrict__ fp_dev, int BH, int vec)
@@ -539,42 +567,67 @@ __global__ void __launch_bounds__(32, 8) k_resample(const float* __restrict__ in
     it.w = w; it.h = h; it.fill = fill;
     it.ax = make_axis(w, sx);
     it.ay = make_axis(h, sy);
-    it.XA = (int)blockIdx.x * OUTCOLS - V * HALO_L;
+    it.XA = (int)blockIdx.x * ModeGeom<MODE>::OUTC - V * ModeGeom<MODE>::HL;
     it.ya = (int)blockIdx.y * BH;
     it.yb = min(it.ya + BH, h);
-    if (fp_dev && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
+    if (MODE != 1 && fp_dev && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
         fp_dev[k] = make_int4(it.ax.lo, it.ax.hi, it.ay.lo, it.ay.hi);
-    if (vec) warp_item<true>(it, s_ring, threadIdx.x);
-    else warp_item<false>(it, s_ring, threadIdx.x);
+    if (vec) warp_item<true, MODE>(it, s_ring, threadIdx.x);
+    else warp_item<false, MODE>(it, s_ring, threadIdx.x);
 }
 
-int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,
-                    const double* dshift_dev, float fill, float* out, int32_t* fp_dev, cudaStream_t st)
+// band height for the kernels that carry y state: enough warps for 148 SMs x 8, no band under 64 rows
+static int band_rows(long long cols, int h)
 {
-    HostShifts hs;
-    if (!dshift_dev)
-        for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
-    const int strips = (w + OUTCOLS - 1) / OUTCOLS;
-    // bands: enough warps to fill 148 SMs x 8 resident warps, but no band shorter than 64 rows
-    // (each band pays ~42 extra rows of warm-up and look-ahead)
-    const long long cols = (long long)strips * n;
     long long bands = (148 * 8 + cols - 1) / cols;
     const long long maxb = (h + 63) / 64;
     if (bands > maxb) bands = maxb;
     if (bands < 1) bands = 1;
     int BH = (int)((h + bands - 1) / bands);
-    BH = (BH + 7) / 8 * 8;
-    const int nb = (h + BH - 1) / BH;
+    return (BH + 7) / 8 * 8;
+}
+
+size_t resample_ws_bytes(int w, int h, int n)
+{
+    const size_t b = (size_t)n * w * h * sizeof(float);
+    return b <= RESAMPLE_TWO_PASS_MAX ? b : 0;
+}
+
+int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,
+                    const double* dshift_dev, float fill, float* out, int32_t* fp_dev, void* ws, size_t ws_bytes,
+                    cudaStream_t st)
+{
+    HostShifts hs;
+    if (!dshift_dev)
+        for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
     const int vec = (w % 4 == 0) ? 1 : 0;
     const size_t smem = (size_t)NRING * RB * WARPCOLS * sizeof(float);
     static bool attr_done = false;   // idempotent: the same value every time, so a race is harmless
     if (!attr_done) {
-        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         attr_done = true;
     }
-    dim3 grid(strips, nb, n);
-    k_resample<<<grid, 32, smem, st>>>(in, n, w, h, hs, dshift_dev, fill, out, reinterpret_cast<int4*>(fp_dev), BH, vec);
+    int4* fpd = reinterpret_cast<int4*>(fp_dev);
+    const size_t need = resample_ws_bytes(w, h, n);
+    if (need && ws && ws_bytes >= need) {
+        // small stack: x pass and y pass as two kernels, the x-shifted rows stay in the 126 MB L2 in between;
+        // neither kernel carries the other's state, so both run with far more parallel work items
+        float* tmp = static_cast<float*>(ws);
+        const int sx1 = (w + ModeGeom<1>::OUTC - 1) / ModeGeom<1>::OUTC, BH1 = 32;
+        k_resample<1><<<dim3(sx1, (h + BH1 - 1) / BH1, n), 32, 0, st>>>(in, n, w, h, hs, dshift_dev, fill, tmp, nullptr, BH1, vec);
+        MRED_LAUNCH_CHECK();
+        const int sx2 = (w + ModeGeom<2>::OUTC - 1) / ModeGeom<2>::OUTC;
+        const int BH2 = band_rows((long long)sx2 * n, h);
+        k_resample<2><<<dim3(sx2, (h + BH2 - 1) / BH2, n), 32, smem, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2, vec);
+        MRED_LAUNCH_CHECK();
+        return MRED_OK;
+    }
+    const int strips = (w + OUTCOLS - 1) / OUTCOLS;
+    const int BH = band_rows((long long)strips * n, h);
+    k_resample<0><<<dim3(strips, (h + BH - 1) / BH, n), 32, smem, st>>>(in, n, w, h, hs, dshift_dev, fill, out, fpd, BH, vec);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
