@@ -72,7 +72,8 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
 #pragma unroll
     for (int k = 0; k < NMAX; ++k) {
         const bool ok = (inside[k >> 5] >> (k & 31)) & 1u;
-        v[k] = ok ? __ldcs(src + (size_t)k * np) : ABSENT;
+        v[k] = ok ? __ldcs(src) : ABSENT;
+        src += np;
     }
     Combined r;
     uint32_t rej[(NMAX + 31) / 32];

@@ -97,6 +97,19 @@ __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict_
 
 // deterministic block sum of one double per thread (256 threads): shuffle tree, then warp 0 adds the
 // eight warp totals in index order.  Result valid in thread 0.
+__device__ __forceinline__ double block_sum_256f(float v, double* s8)
+{
+    v = warp_sum(v);          // 32 lanes x <= 2 pixels in float32: relative error 1e-6 of a block partial, far below
+                              // what <MB>, <MD>, <MF> need (they enter <G_k> ~ 2e4 ADU to 1e-7 relative)
+    if ((threadIdx.x & 31) == 0) s8[threadIdx.x >> 5] = (double)v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < 8; ++i) t += s8[i];
+    __syncthreads();
+    return t;
+}
+
 __device__ __forceinline__ double block_sum_256(double v, double* s8)
 {
     v = warp_sum(v);
@@ -168,19 +181,23 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
         const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
         const size_t p = (size_t)y * g.w + x;
         float v[PX][NMAX];
+        const uint16_t* pb = bias + q;
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX];
-            if (k < nb) load_px<PX>(bias + (size_t)k * fs, q, nv, o);
+            if (k < nb) load_px<PX>(pb, 0, nv, o);
+            pb += fs;
 #pragma unroll
             for (int i = 0; i < PX; ++i) v[i][k] = k < nb ? o[i] - s_lb[k] : ABSENT;
         }
 #pragma unroll
         for (int i = 0; i < PX; ++i) mb[i] = combine_all<NMAX, MODE>(v[i], nb, ksigma, max_iter);
+        const uint16_t* pd = dark + q;
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX];
-            if (k < nd) load_px<PX>(dark + (size_t)k * fs, q, nv, o);
+            if (k < nd) load_px<PX>(pd, 0, nv, o);
+            pd += fs;
 #pragma unroll
             for (int i = 0; i < PX; ++i) v[i][k] = k < nd ? (o[i] - s_ld[k]) - mb[i] : ABSENT;
         }
@@ -196,11 +213,11 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
         for (int i = 0; i < PX; ++i)
             if (i >= nv) { mb[i] = 0.f; md[i] = 0.f; }
     }
-    double tb = 0.0, td = 0.0;
+    float tb = 0.f, td = 0.f;
 #pragma unroll
-    for (int i = 0; i < PX; ++i) { tb += (double)mb[i]; td += (double)md[i]; }
-    const double sb = block_sum_256(tb, s8);
-    const double sd = block_sum_256(td, s8);
+    for (int i = 0; i < PX; ++i) { tb += mb[i]; td += md[i]; }
+    const double sb = block_sum_256f(tb, s8);
+    const double sd = block_sum_256f(td, s8);
     if (threadIdx.x == 0) { m.part_bd[2 * (size_t)blockIdx.x] = sb; m.part_bd[2 * (size_t)blockIdx.x + 1] = sd; }
     if (!last_block(m.ticket)) return;
     // <G_k> = <F_k> - L_k - <MB> - r <MD>: fixed-order sums of the block partials
@@ -249,10 +266,12 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
 #pragma unroll
         for (int i = 0; i < PX; ++i) off[i] = i < nv ? fmaf(r, MD[p + i], MB[p + i]) : 0.f;
         float v[PX][NMAX];
+        const uint16_t* pf = flat + q;
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX];
-            if (k < nf) load_px<PX>(flat + (size_t)k * fs, q, nv, o);
+            if (k < nf) load_px<PX>(pf, 0, nv, o);
+            pf += fs;
 #pragma unroll
             for (int i = 0; i < PX; ++i) v[i][k] = k < nf ? ((o[i] - s_lf[k]) - off[i]) * s_ig[k] : ABSENT;
         }
@@ -264,10 +283,10 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
         for (int i = 0; i < PX; ++i)
             if (i >= nv) mf[i] = 0.f;
     }
-    double t = 0.0;
+    float t = 0.f;
 #pragma unroll
-    for (int i = 0; i < PX; ++i) t += (double)mf[i];
-    const double sblk = block_sum_256(t, s8);
+    for (int i = 0; i < PX; ++i) t += mf[i];
+    const double sblk = block_sum_256f(t, s8);
     if (threadIdx.x == 0) m.part_f[blockIdx.x] = sblk;
     if (!last_block(m.ticket + 1)) return;
     double a = 0.0;

@@ -577,10 +577,10 @@ __global__ void __launch_bounds__(32, MODE == 1 ? 16 : 8) k_resample(const float
 }
 
 // band height for the kernels that carry y state: enough warps for 148 SMs x 8, no band under 64 rows
-static int band_rows(long long cols, int h)
+static int band_rows(long long cols, int h, int min_rows = 64)
 {
     long long bands = (148 * 8 + cols - 1) / cols;
-    const long long maxb = (h + 63) / 64;
+    const long long maxb = (h + min_rows - 1) / min_rows;
     if (bands > maxb) bands = maxb;
     if (bands < 1) bands = 1;
     int BH = (int)((h + bands - 1) / bands);
@@ -616,11 +616,14 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
         // small stack: x pass and y pass as two kernels, the x-shifted rows stay in the 126 MB L2 in between;
         // neither kernel carries the other's state, so both run with far more parallel work items
         float* tmp = static_cast<float*>(ws);
-        const int sx1 = (w + ModeGeom<1>::OUTC - 1) / ModeGeom<1>::OUTC, BH1 = 32;
+        const int sx1 = (w + ModeGeom<1>::OUTC - 1) / ModeGeom<1>::OUTC;
+        int BH1 = (int)(((long long)h * sx1 * n + 148 * 16 - 1) / (148 * 16));     // one wave of 16 warps per SM
+        BH1 = (BH1 + 3) / 4 * 4;
+        if (BH1 < 8) BH1 = 8;
         k_resample<1><<<dim3(sx1, (h + BH1 - 1) / BH1, n), 32, 0, st>>>(in, n, w, h, hs, dshift_dev, fill, tmp, nullptr, BH1, vec);
         MRED_LAUNCH_CHECK();
         const int sx2 = (w + ModeGeom<2>::OUTC - 1) / ModeGeom<2>::OUTC;
-        const int BH2 = band_rows((long long)sx2 * n, h);
+        const int BH2 = band_rows((long long)sx2 * n, h, 48);
         k_resample<2><<<dim3(sx2, (h + BH2 - 1) / BH2, n), 32, smem, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2, vec);
         MRED_LAUNCH_CHECK();
         return MRED_OK;
