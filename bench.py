@@ -180,10 +180,10 @@ def run_reference(args):
     cfg = args.config
     plan = oracle_sample_plan(cfg)
     grp = synth.make_group(cfg, 0, **plan)
-    steps = max(1, min(args.steps, 3))
-    warm = 1 if args.warmup > 0 else 0
+    steps = max(1, args.steps)                 # exactly K timed steps; one step = the bounded sample (~1 s at config 2)
+    warm = max(0, args.warmup)
     for _ in range(warm):
-        time_oracle_group(grp, MAX_LAG[cfg], n_sci=2)
+        time_oracle_group(grp, MAX_LAG[cfg])
     tot, frames = 0.0, 0
     for _ in range(steps):
         s, n, _ = time_oracle_group(grp, MAX_LAG[cfg])
@@ -205,7 +205,7 @@ def run_reference(args):
 # GPU arm
 # ------------------------------------------------------------------------------------------------
 KERNELS_PER_BUILD_MASTERS = 4    # k_master_sums, k_masters_bd, k_masters_f, k_mf_scale
-KERNELS_PER_REDUCE = 6           # k_frame_sums, k_calibrate, k_profiles, k_shifts, k_resample, k_coadd
+KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd (+1: small stacks resample in two kernels)
 
 
 def run_ours(args):
@@ -381,7 +381,7 @@ def run_ours(args):
             gbs = sb[k] / (ms * 1e-3) / 1e9
             stages_iso[k] = {"ms_per_call": round(ms, 5), "GBps": round(gbs, 1), "frac": round(gbs / peak, 4)}
     dom = max(STAGES, key=lambda k: np.sum(st_ms[k]))
-    kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_shifts)",
+    kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_finalize, k_correlate)",
             "resample": "k_resample", "coadd": "k_coadd"}[dom]
     traffic = None
     tr_path = os.path.join(ROOT, "profiles", "traffic.json")      # ncu --set full capture of config 2 (profiles/r1f_kernels.md)
@@ -451,7 +451,7 @@ def run_ours(args):
                            "coadd": ["median", "mean", "sigclip 3.0 x3"][mode], "l2": "512 MB flush before every step",
                            "parallelism": "groups sharded over ranks, no collective", "streams": len(streams), "launch": "cuda graph replay" if graph is not None else "plain launches",
                            "stage_timing": "CUDA events inside the C call; with a graph: instrumented plain-launch passes of the same step right after the timed region"},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + KERNELS_PER_REDUCE),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + KERNELS_PER_REDUCE + (1 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 0)),
                 "roofline": roof, "stages": stages, "stages_isolated": stages_iso, "path_roofline": e2e_roof, "cpu_baseline": cpu,
                 "wall_s_timed_region": round(wall, 4), "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU "
                 "stages on a TITAN X (Pascal) = ~870 frames/s (other hardware, other data; context only)"}

@@ -4,8 +4,8 @@
 //
 //   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): float64 column
 //                partial sums per 64-row band and complete float64 row sums, valid-pixel counts.
-//   k_shifts   : per (frame, axis): fixed-order band sum, mean, median by a shared-memory radix select, subtract
-//                (for the reference and for the frame), then C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
+//   k_finalize : per (frame, axis): fixed-order band sum, mean, median by a shared-memory radix select, subtract.
+//   k_correlate: per (frame, axis): C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
 //                smaller |l| then smaller l; 3-point parabola.
 // No float atomics: every sum has a fixed order, so the integer result is reproducible.
 #include "common.cuh"
@@ -206,7 +206,8 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
         }
         keys[i] = key_of(v);
     }
-    if (mine) atomicAdd(s_m, mine);
+    mine = warp_sum(mine);                     // one shared-memory atomic per warp, not per thread:
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(s_m, mine);   // 1024 same-address atomics cost ~15 us
     __syncthreads();
     const int m = *s_m;
     double med = 0.0;
@@ -246,29 +247,42 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
     __syncthreads();
 }
 
-// grid (n, 2), block 1024: block (k, axis) builds the reference profile and its own (each block redoes the
-// reference: 2n tiny blocks run in parallel, and no block waits for another), then the 2R+1 lags, one per warp
-// and round, from shared memory; argmax with ties to the smaller |l| then smaller l; 3-point parabola.
-__global__ void __launch_bounds__(1024) k_shifts(int w, int h, int n, int ref, int R, EstimateWs e,
-                                                 int32_t* __restrict__ ishift, double* __restrict__ shift)
+// grid (n, 2), block 1024: median-subtracted mean profile of (frame, axis) -> e.prof
+__global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
 {
-    extern __shared__ double s_dyn[];     // a[P], b[P], selection keys[P]
-    __shared__ double s_C[2 * MRED_MAX_LAG + 1];
+    extern __shared__ double s_dyn[];     // profile[P], selection keys[P]
     __shared__ SelectScratch s_sc;
     __shared__ int s_m;
+    const int k = blockIdx.x, axis = blockIdx.y;
+    const int len = axis == 0 ? w : h;
+    int P = 1;
+    while (P < len) P <<= 1;
+    double* a = s_dyn;
+    unsigned long long* keys = reinterpret_cast<unsigned long long*>(s_dyn + P);
+    block_profile(e, w, h, k, axis, len, P, a, keys, &s_sc, &s_m);
+    double* out = e.prof + ((size_t)k * 2 + axis) * e.plen;
+    for (int i = threadIdx.x; i < len; i += blockDim.x) out[i] = a[i];
+}
+
+// grid (n, 2), block 1024: C(l) = sum_j a[j] b[j+l] for the 2R+1 lags, one per warp and round, both profiles
+// staged in shared memory; argmax with ties to the smaller |l| then smaller l; 3-point parabola.
+__global__ void __launch_bounds__(1024) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
+                                                    int32_t* __restrict__ ishift, double* __restrict__ shift)
+{
+    extern __shared__ double s_dyn[];     // a[len], b[len]
+    __shared__ double s_C[2 * MRED_MAX_LAG + 1];
     const int k = blockIdx.x, axis = blockIdx.y;
     if (k == ref) {
         if (threadIdx.x == 0) { ishift[2 * k + axis] = 0; shift[2 * k + axis] = 0.0; }
         return;
     }
     const int len = axis == 0 ? w : h;
-    int P = 1;
-    while (P < len) P <<= 1;
     double* a = s_dyn;
-    double* b = s_dyn + P;
-    unsigned long long* keys = reinterpret_cast<unsigned long long*>(s_dyn + 2 * P);
-    block_profile(e, w, h, ref, axis, len, P, a, keys, &s_sc, &s_m);
-    block_profile(e, w, h, k, axis, len, P, b, keys, &s_sc, &s_m);
+    double* b = s_dyn + len;
+    const double* ga = e.prof + ((size_t)ref * 2 + axis) * e.plen;
+    const double* gb = e.prof + ((size_t)k * 2 + axis) * e.plen;
+    for (int i = threadIdx.x; i < len; i += blockDim.x) { a[i] = ga[i]; b[i] = gb[i]; }
+    __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int l = -R + warp; l <= R; l += 32) {
         const int j0 = max(0, -l), j1 = min(len, len - l);
@@ -309,13 +323,15 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     MRED_LAUNCH_CHECK();
     int P = 1;
     while (P < (w > h ? w : h)) P <<= 1;
-    const size_t smem = 3 * (size_t)P * sizeof(double);
     static bool attr_done = false;   // idempotent
     if (!attr_done) {
-        MRED_CUDA_TRY(cudaFuncSetAttribute(k_shifts, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * PROF_MAXLEN * (int)sizeof(double)));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_finalize, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_correlate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
         attr_done = true;
     }
-    k_shifts<<<dim3(n, 2), 1024, smem, st>>>(w, h, n, ref, max_lag, e, ishift, shift);
+    k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, e);
+    MRED_LAUNCH_CHECK();
+    k_correlate<<<dim3(n, 2), 1024, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
