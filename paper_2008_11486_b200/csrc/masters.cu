@@ -68,15 +68,24 @@ __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict_
         unsigned long long s = 0;
         if (r < g.H && g.os_x1 > g.os_x0) s = overscan_row_sum(f, g.W, g.os_x0, g.os_x1, r);
         s = warp_sum(s);
-        if (lane == 0 && s) atomicAdd(os + k, s);
+        __shared__ unsigned long long s_w[8];
+        if (lane == 0) s_w[warp] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long t = 0;
+            for (int i = 0; i < 8; ++i) t += s_w[i];
+            if (t) atomicAdd(os + k, t);
+        }
         return;
     }
     if (k < nb + nd) return;                       // image sums: flats only
     const int r = g.y0 + ((int)blockIdx.x - nos) * 8 + warp;
-    if (r >= g.y0 + g.h) return;
-    const uint16_t* row = f + (size_t)r * g.W;
+    __shared__ unsigned long long s_b[8];
+    const bool live = r < g.y0 + g.h;
+    const uint16_t* row = f + (size_t)(live ? r : g.y0) * g.W;
     unsigned long long b = 0;
-    if (pair_ok) {      // two pixels per 32-bit load, 8 independent loads in flight
+    if (!live) {
+    } else if (pair_ok) {      // two pixels per 32-bit load, 8 independent loads in flight
         const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
         const int w2 = g.w >> 1;
         int x = lane;
@@ -92,7 +101,13 @@ __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict_
         for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
     }
     b = warp_sum(b);
-    if (lane == 0 && b) atomicAdd(img_f + (k - nb - nd), b);
+    if (lane == 0) s_b[warp] = b;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int i = 0; i < 8; ++i) t += s_b[i];
+        if (t) atomicAdd(img_f + (k - nb - nd), t);
+    }
 }
 
 // deterministic block sum of one double per thread (256 threads): shuffle tree, then warp 0 adds the
@@ -180,26 +195,27 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
         const int nv = min(PX, g.w - x);
         const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
         const size_t p = (size_t)y * g.w + x;
-        float v[PX][NMAX];
+        float v[PX][NMAX], dk[PX][NMAX];
         const uint16_t* pb = bias + q;
+        const uint16_t* pd = dark + q;
+        // every load of both stacks is issued before the first median starts
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
-            float o[PX];
-            if (k < nb) load_px<PX>(pb, 0, nv, o);
-            pb += fs;
+            float o[PX], od[PX];
 #pragma unroll
-            for (int i = 0; i < PX; ++i) v[i][k] = k < nb ? o[i] - s_lb[k] : ABSENT;
+            for (int i = 0; i < PX; ++i) { o[i] = 0.f; od[i] = 0.f; }
+            if (k < nb) load_px<PX>(pb, 0, nv, o);
+            if (k < nd) load_px<PX>(pd, 0, nv, od);
+            pb += fs; pd += fs;
+#pragma unroll
+            for (int i = 0; i < PX; ++i) { v[i][k] = k < nb ? o[i] - s_lb[k] : ABSENT; dk[i][k] = od[i]; }
         }
 #pragma unroll
         for (int i = 0; i < PX; ++i) mb[i] = combine_all<NMAX, MODE>(v[i], nb, ksigma, max_iter);
-        const uint16_t* pd = dark + q;
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
-            float o[PX];
-            if (k < nd) load_px<PX>(pd, 0, nv, o);
-            pd += fs;
 #pragma unroll
-            for (int i = 0; i < PX; ++i) v[i][k] = k < nd ? (o[i] - s_ld[k]) - mb[i] : ABSENT;
+            for (int i = 0; i < PX; ++i) v[i][k] = k < nd ? (dk[i][k] - s_ld[k]) - mb[i] : ABSENT;
         }
 #pragma unroll
         for (int i = 0; i < PX; ++i) md[i] = combine_all<NMAX, MODE>(v[i], nd, ksigma, max_iter);
