@@ -158,10 +158,13 @@ def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stre
 
 def resample(frames, sx, sy, fill=0.0, out=None, ws=None, stream=None):
     """include/mred.h: mred_resample.  sx, sy: host float64 [n].  Returns (out, footprint int32 [n][4] numpy).
-    ws: optional scratch of workspace_bytes(CALL_RESAMPLE, ...) bytes (allocated here when None and non-zero)."""
+    ws: optional scratch of workspace_bytes(CALL_RESAMPLE, ...) bytes (allocated here when None and non-zero);
+    ws=False passes no workspace, which selects the one-kernel route whatever the stack size."""
     n, h, w = frames.shape
     need = workspace_bytes(CALL_RESAMPLE, Geom(0, 0, 0, 0, 0, 0, w, h), n)
-    if ws is None and need:
+    if ws is False:
+        ws = None
+    elif ws is None and need:
         ws = torch.empty(need, dtype=torch.uint8, device=frames.device)
     sx = np.ascontiguousarray(np.broadcast_to(np.asarray(sx, np.float64), (n,)))
     sy = np.ascontiguousarray(np.broadcast_to(np.asarray(sy, np.float64), (n,)))

@@ -263,6 +263,28 @@ def test_resample_parity(shape):
     assert np.array_equal(got[0], img[0])                      # zero shift = bit-exact identity
 
 
+def test_resample_both_routes():
+    """mred_resample has two routes (include/mred.h): x kernel + y kernel through the workspace (small stacks), and
+    one fused kernel (no workspace, large stacks).  Both against the oracle on the same input, integer shifts exact."""
+    h, w = 216, 424
+    rng = np.random.default_rng(5)
+    n = len(SHIFTS)
+    img = rng.normal(1000, 30, size=(n, h, w)).astype(np.float32)
+    img[rng.random(img.shape) < 0.002] = 65535.0
+    sx = np.array([s[0] for s in SHIFTS])
+    sy = np.array([s[1] for s in SHIFTS])
+    ref = oracle.resample(img, sx, sy, fill=7.0)
+    assert mred.workspace_bytes(mred.CALL_RESAMPLE, Geom(0, 0, 0, 0, 0, 0, w, h), n) == img.nbytes
+    two, fp2 = mred.resample(dev(img), sx, sy, fill=7.0)                 # workspace allocated by the binding
+    one, fp1 = mred.resample(dev(img), sx, sy, fill=7.0, ws=False)       # fused kernel
+    assert np.array_equal(fp1, ref.footprint) and np.array_equal(fp2, ref.footprint)
+    assert_close(host(two), ref.out, "resample two-kernel route", local=4)
+    assert_close(host(one), ref.out, "resample fused route", local=4)
+    for k, (a, b) in enumerate(SHIFTS):
+        if a == np.floor(a) and b == np.floor(b):
+            assert np.array_equal(host(two)[k], ref.out[k]) and np.array_equal(host(one)[k], ref.out[k])
+
+
 def test_resample_bspline_image_matches_paper_precision(golden):
     """float32 spline shift of the B-spline-basis image differs from the analytic
     reference by about 1e-7."""
@@ -345,6 +367,15 @@ def test_config1_full_size_stage_isolated():
     assert_close(host(reg), r.out, "resample", local=4)
     _compare_coadd(r.out, r.footprint, 0)
     _compare_coadd(r.out, r.footprint, 2)
+
+
+def test_config2_group_full_size_chained():
+    """BASELINE.json config 2 (the bench workload): one group at full size through mred_build_masters + mred_reduce,
+    exactly the calls and launch configuration bench.py times (10 frames: two-kernel resample route, N = 10 buckets)."""
+    grp = synth.make_group(2, 1)
+    e = _chain_check(grp, 32, 2)
+    assert np.array_equal(np.rint(e.shift), np.rint(grp.shifts))          # diagnostic: integer part of the truth
+    assert np.max(np.abs(e.shift - grp.shifts)) < 0.05
 
 
 def test_config4_stress_coadd_full_size():
