@@ -205,7 +205,7 @@ def run_reference(args):
 # GPU arm
 # ------------------------------------------------------------------------------------------------
 KERNELS_PER_BUILD_MASTERS = 4    # k_master_sums, k_masters_bd, k_masters_f, k_mf_scale
-KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd (+1: small stacks resample in two kernels)
+KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd (+1: small stacks resample in two kernels); memset nodes not counted
 
 
 def run_ours(args):

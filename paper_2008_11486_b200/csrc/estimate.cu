@@ -2,8 +2,8 @@
 // The paper obtains relative positions from FITS WCS headers on the CPU;
 // with no headers here the north star asks for an image-based estimate.
 //
-//   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): float64 column
-//                partial sums per 64-row band and complete float64 row sums, valid-pixel counts.
+//   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): fixed-point (int64) column
+//                partial sums per 32-row band and complete row sums, valid-pixel counts.
 //   k_finalize : per (frame, axis): fixed-order band sum, mean, median by a shared-memory radix select, subtract.
 //   k_correlate: per (frame, axis): C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
 //                smaller |l| then smaller l; 3-point parabola.
@@ -13,14 +13,17 @@
 namespace mred {
 
 constexpr int PROF_BR = 32;        // rows per band
+constexpr float FIX = 16384.0f;    // fixed-point scale of the profile sums (2^14: 6e-5 ADU per partial)
 constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
 
 struct EstimateWs {
-    double* colpart;  // [n][nbands][w]
+    long long* colpart;  // [n][nbands][w]   fixed-point sums (value * FIX, see k_profiles)
     int* colcnt;      // [n][nbands][w]
-    double* rowsum;   // [n][h]
+    long long* rowsum;   // [n][h]
     int* rowcnt;      // [n][h]
     double* prof;     // [n][2][plen]  median-subtracted profiles (x then y)
+    double* corr;     // [n][2][2*MRED_MAX_LAG+1]  C(l) of every lag
+    unsigned int* ticket;  // [n][2] block counters of k_correlate (zeroed per call)
     size_t bytes;
     int nbands, plen;
 };
@@ -32,11 +35,13 @@ static EstimateWs carve_est(void* ws, int w, int h, int n)
     auto take = [&](size_t b) { char* q = p; p += align_up(b, 16); return q; };
     e.nbands = (h + PROF_BR - 1) / PROF_BR;
     e.plen = w > h ? w : h;
-    e.colpart = reinterpret_cast<double*>(take(8 * (size_t)n * e.nbands * w));
+    e.colpart = reinterpret_cast<long long*>(take(8 * (size_t)n * e.nbands * w));
     e.colcnt = reinterpret_cast<int*>(take(4 * (size_t)n * e.nbands * w));
-    e.rowsum = reinterpret_cast<double*>(take(8 * (size_t)n * h));
+    e.rowsum = reinterpret_cast<long long*>(take(8 * (size_t)n * h));
     e.rowcnt = reinterpret_cast<int*>(take(4 * (size_t)n * h));
     e.prof = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * e.plen));
+    e.corr = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * (2 * MRED_MAX_LAG + 1)));
+    e.ticket = reinterpret_cast<unsigned int*>(take(4 * (size_t)n * 2));
     e.bytes = (size_t)(p - static_cast<char*>(ws));
     return e;
 }
@@ -46,18 +51,18 @@ size_t estimate_ws_bytes(int w, int h, int n) { return carve_est(nullptr, w, h, 
 __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ frames, int w, int h,
                                                   const uint8_t* __restrict__ bad, EstimateWs e, int vec_ok)
 {
-    __shared__ double s_row[PROF_BR][8];
+    __shared__ long long s_row[PROF_BR][8];
     __shared__ int s_cnt[PROF_BR][8];
     const int band = blockIdx.x, k = blockIdx.y;
     const int y0 = band * PROF_BR, y1 = min(y0 + PROF_BR, h);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const float* f = frames + (size_t)k * w * h;
-    for (int i = threadIdx.x; i < PROF_BR * 8; i += blockDim.x) { (&s_row[0][0])[i] = 0.0; (&s_cnt[0][0])[i] = 0; }
+    for (int i = threadIdx.x; i < PROF_BR * 8; i += blockDim.x) { (&s_row[0][0])[i] = 0; (&s_cnt[0][0])[i] = 0; }
     __syncthreads();
     for (int xc = 0; xc < w; xc += 1024) {
         const int x = xc + 4 * threadIdx.x;
         const int nv = max(0, min(4, w - x));
-        double cs[4] = {0.0, 0.0, 0.0, 0.0};
+        long long cs[4] = {0, 0, 0, 0};
         int cc[4] = {0, 0, 0, 0};
         for (int yb = y0; yb < y1; yb += 4) {       // 4 rows in flight per thread
             float v[4][4];
@@ -81,13 +86,18 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
                     for (int i = 0; i < nv; ++i) { v[u][i] = __ldcs(f + p + i); ok[u][i] = bad ? !__ldg(bad + p + i) : true; }
                 }
             }
-            double rs[4] = {0.0, 0.0, 0.0, 0.0};
+            // Vector FP64 is a few lanes per SM on this part, so no float64 in the streaming loop: 4 rows are summed in
+            // float32 (relative error 6e-8 of a 4-value sum), then accumulated as 64-bit fixed point (value * 2^14):
+            // integer adds are exact and order-independent, so the profile is reproducible bit for bit.
+            float c4[4] = {0.f, 0.f, 0.f, 0.f}, rs[4] = {0.f, 0.f, 0.f, 0.f};
             int rc[4] = {0, 0, 0, 0};
 #pragma unroll
             for (int u = 0; u < 4; ++u)
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
-                    if (ok[u][i]) { const double d = (double)v[u][i]; cs[i] += d; ++cc[i]; rs[u] += d; ++rc[u]; }
+                    if (ok[u][i]) { c4[i] += v[u][i]; ++cc[i]; rs[u] += v[u][i]; ++rc[u]; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) cs[i] += __float2ll_rn(c4[i] * FIX);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
@@ -95,7 +105,7 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
             if (lane == 0) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (yb + u < y1) { s_row[yb + u - y0][warp] += rs[u]; s_cnt[yb + u - y0][warp] += rc[u]; }
+                    if (yb + u < y1) { s_row[yb + u - y0][warp] += __float2ll_rn(rs[u] * FIX); s_cnt[yb + u - y0][warp] += rc[u]; }
             }
         }
         for (int i = 0; i < nv; ++i) {
@@ -105,7 +115,7 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
     }
     __syncthreads();
     for (int r = threadIdx.x; r < y1 - y0; r += blockDim.x) {
-        double t = 0.0;
+        long long t = 0;
         int c = 0;
         for (int i = 0; i < 8; ++i) { t += s_row[r][i]; c += s_cnt[r][i]; }
         e.rowsum[(size_t)k * h + y0 + r] = t;
@@ -137,13 +147,18 @@ __device__ unsigned long long block_select(const unsigned long long* keys, int P
         __syncthreads();
         const unsigned long long prefix = sc->prefix;
         for (int i = threadIdx.x; i < P; i += blockDim.x) {
-            // profile values share their leading bytes, so a pass would send a whole warp to one bin:
-            // aggregate equal digits inside the warp first (one shared-memory atomic per distinct digit)
+            // profile values share their leading bytes, so in the first passes a whole warp hits ONE bin: count such a
+            // warp with a single atomic (vote, not __match_any_sync: MATCH costs hundreds of cycles per call here)
             const unsigned long long k = keys[i];
             const unsigned int am = __activemask();
             const unsigned int d = ((k & mask) == prefix) ? ((unsigned int)(k >> shift) & 255u) : 256u;
-            const unsigned int same = __match_any_sync(am, d);
-            if (d < 256u && (threadIdx.x & 31) == (unsigned int)(__ffs(same) - 1)) atomicAdd(&sc->hist[d], (unsigned int)__popc(same));
+            const int leader = __ffs(am) - 1;
+            const unsigned int d0 = __shfl_sync(am, d, leader);
+            if (__all_sync(am, d == d0)) {
+                if ((int)(threadIdx.x & 31) == leader && d < 256u) atomicAdd(&sc->hist[d], (unsigned int)__popc(am));
+            } else if (d < 256u) {
+                atomicAdd(&sc->hist[d], 1u);
+            }
         }
         __syncthreads();
         if (threadIdx.x < 32) {          // warp 0: find the bin that holds the rank (8 bins per lane)
@@ -182,26 +197,26 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
     for (int i = threadIdx.x; i < P; i += blockDim.x) {
         double v = INF;
         if (i < len) {
-            double s = 0.0;
+            long long s = 0;
             int c = 0;
             if (axis == 0) {
-                const double* cp = e.colpart + (size_t)k * e.nbands * w + i;
+                const long long* cp = e.colpart + (size_t)k * e.nbands * w + i;
                 const int* cc = e.colcnt + (size_t)k * e.nbands * w + i;
                 int b = 0;
-                for (; b + 8 <= e.nbands; b += 8) {          // 8 bands in flight; the order of the adds stays fixed
-                    double tv[8];
+                for (; b + 8 <= e.nbands; b += 8) {          // 8 bands in flight
+                    long long tv[8];
                     int tc[8];
 #pragma unroll
-                    for (int u = 0; u < 8; ++u) { tv[u] = __ldcg(cp + (size_t)(b + u) * w); tc[u] = __ldcg(cc + (size_t)(b + u) * w); }
+                    for (int u = 0; u < 8; ++u) { tv[u] = __ldg(cp + (size_t)(b + u) * w); tc[u] = __ldg(cc + (size_t)(b + u) * w); }
 #pragma unroll
                     for (int u = 0; u < 8; ++u) { s += tv[u]; c += tc[u]; }
                 }
-                for (; b < e.nbands; ++b) { s += __ldcg(cp + (size_t)b * w); c += __ldcg(cc + (size_t)b * w); }
+                for (; b < e.nbands; ++b) { s += __ldg(cp + (size_t)b * w); c += __ldg(cc + (size_t)b * w); }
             } else {
-                s = __ldcg(e.rowsum + (size_t)k * h + i);
-                c = __ldcg(e.rowcnt + (size_t)k * h + i);
+                s = __ldg(e.rowsum + (size_t)k * h + i);
+                c = __ldg(e.rowcnt + (size_t)k * h + i);
             }
-            if (c > 0) { v = s / (double)c; ++mine; }
+            if (c > 0) { v = (double)s / ((double)FIX * (double)c); ++mine; }
             dst[i] = v;
         }
         keys[i] = key_of(v);
@@ -264,16 +279,19 @@ __global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
     for (int i = threadIdx.x; i < len; i += blockDim.x) out[i] = a[i];
 }
 
-// grid (n, 2), block 1024: C(l) = sum_j a[j] b[j+l] for the 2R+1 lags, one per warp and round, both profiles
-// staged in shared memory; argmax with ties to the smaller |l| then smaller l; 3-point parabola.
-__global__ void __launch_bounds__(1024) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
-                                                    int32_t* __restrict__ ishift, double* __restrict__ shift)
+// grid (n, 2, CORR_Z), block 256: C(l) = sum_j a[j] b[j+l] (float64: the one place it is kept, ~65 k DFMA per
+// profile pair, spread over CORR_Z blocks because vector FP64 is scarce per SM), both profiles staged in shared
+// memory, lags dealt round-robin to the warps of the CORR_Z blocks; the last block of a (frame, axis) to finish
+// takes the argmax (ties: smaller |l|, then smaller l) and the 3-point parabola.
+constexpr int CORR_Z = 8;
+__global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
+                                                   int32_t* __restrict__ ishift, double* __restrict__ shift)
 {
     extern __shared__ double s_dyn[];     // a[len], b[len]
-    __shared__ double s_C[2 * MRED_MAX_LAG + 1];
+    __shared__ int s_last;
     const int k = blockIdx.x, axis = blockIdx.y;
     if (k == ref) {
-        if (threadIdx.x == 0) { ishift[2 * k + axis] = 0; shift[2 * k + axis] = 0.0; }
+        if (threadIdx.x == 0 && blockIdx.z == 0) { ishift[2 * k + axis] = 0; shift[2 * k + axis] = 0.0; }
         return;
     }
     const int len = axis == 0 ? w : h;
@@ -284,34 +302,43 @@ __global__ void __launch_bounds__(1024) k_correlate(int w, int h, int n, int ref
     for (int i = threadIdx.x; i < len; i += blockDim.x) { a[i] = ga[i]; b[i] = gb[i]; }
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int l = -R + warp; l <= R; l += 32) {
+    double* C = e.corr + ((size_t)k * 2 + axis) * (2 * MRED_MAX_LAG + 1);
+    for (int q = (int)blockIdx.z + CORR_Z * warp; q <= 2 * R; q += CORR_Z * 8) {
+        const int l = q - R;
         const int j0 = max(0, -l), j1 = min(len, len - l);
         double s = 0.0;
         for (int j = j0 + lane; j < j1; j += 32) s = fma(a[j], b[j + l], s);
         s = warp_sum(s);
-        if (lane == 0) s_C[l + R] = s;
+        if (lane == 0) C[q] = s;
     }
+    __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int best = 0;
-        for (int l = -R; l <= R; ++l) {
-            const double c = s_C[l + R], cb = s_C[best + R];
-            const int al = l < 0 ? -l : l, ab = best < 0 ? -best : best;
-            if (c > cb || (c == cb && (al < ab || (al == ab && l < best)))) best = l;
-        }
-        double delta = 0.0;
-        const int ab = best < 0 ? -best : best;
-        if (ab < R) {
-            const double cm = s_C[best - 1 + R], c0 = s_C[best + R], cp = s_C[best + 1 + R];
-            const double den = cm - 2.0 * c0 + cp;
-            if (den < 0.0) {
-                delta = 0.5 * (cm - cp) / den;
-                delta = delta > 0.5 ? 0.5 : (delta < -0.5 ? -0.5 : delta);
-            }
-        }
-        ishift[2 * k + axis] = best;
-        shift[2 * k + axis] = (double)best + delta;
+    if (threadIdx.x == 0) s_last = (atomicAdd(e.ticket + 2 * k + axis, 1u) == CORR_Z - 1);
+    __syncthreads();
+    if (!s_last) return;
+    double* sC = s_dyn;                      // the profiles are no longer needed: reuse their space (2R+1 <= 2 len)
+    __syncthreads();
+    for (int q = threadIdx.x; q <= 2 * R; q += blockDim.x) sC[q] = __ldcg(C + q);
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    int best = 0;
+    for (int l = -R; l <= R; ++l) {
+        const double c = sC[l + R], cb = sC[best + R];
+        const int al = l < 0 ? -l : l, ab = best < 0 ? -best : best;
+        if (c > cb || (c == cb && (al < ab || (al == ab && l < best)))) best = l;
     }
+    double delta = 0.0;
+    const int ab = best < 0 ? -best : best;
+    if (ab < R) {
+        const double cm = sC[best - 1 + R], c0 = sC[best + R], cp = sC[best + 1 + R];
+        const double den = cm - 2.0 * c0 + cp;
+        if (den < 0.0) {
+            delta = 0.5 * (cm - cp) / den;
+            delta = delta > 0.5 ? 0.5 : (delta < -0.5 ? -0.5 : delta);
+        }
+    }
+    ishift[2 * k + axis] = best;
+    shift[2 * k + axis] = (double)best + delta;
 }
 
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
@@ -331,7 +358,8 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     }
     k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, e);
     MRED_LAUNCH_CHECK();
-    k_correlate<<<dim3(n, 2), 1024, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, e, ishift, shift);
+    MRED_CUDA_TRY(cudaMemsetAsync(e.ticket, 0, sizeof(unsigned int) * 2 * (size_t)n, st));
+    k_correlate<<<dim3(n, 2, CORR_Z), 256, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
