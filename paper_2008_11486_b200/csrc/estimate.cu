@@ -13,6 +13,7 @@
 namespace mred {
 
 constexpr int PROF_BR = 32;        // rows per band
+constexpr int RIF = 4;             // rows in flight per thread in k_profiles
 constexpr float FIX = 16384.0f;    // fixed-point scale of the profile sums (2^14: 6e-5 ADU per partial)
 constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
 
@@ -64,11 +65,11 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
         const int nv = max(0, min(4, w - x));
         long long cs[4] = {0, 0, 0, 0};
         int cc[4] = {0, 0, 0, 0};
-        for (int yb = y0; yb < y1; yb += 4) {       // 4 rows in flight per thread
-            float v[4][4];
-            bool ok[4][4];
+        for (int yb = y0; yb < y1; yb += RIF) {     // RIF rows in flight per thread
+            float v[RIF][4];
+            bool ok[RIF][4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < RIF; ++u) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i) { v[u][i] = 0.f; ok[u][i] = false; }
                 const int y = yb + u;
@@ -86,13 +87,15 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
                     for (int i = 0; i < nv; ++i) { v[u][i] = __ldcs(f + p + i); ok[u][i] = bad ? !__ldg(bad + p + i) : true; }
                 }
             }
-            // Vector FP64 is a few lanes per SM on this part, so no float64 in the streaming loop: 4 rows are summed in
-            // float32 (relative error 6e-8 of a 4-value sum), then accumulated as 64-bit fixed point (value * 2^14):
+            // No float64 in the streaming loop: RIF rows are summed in
+            // float32 (relative error 6e-8 of an 8-value sum), then accumulated as 64-bit fixed point (value * 2^14):
             // integer adds are exact and order-independent, so the profile is reproducible bit for bit.
-            float c4[4] = {0.f, 0.f, 0.f, 0.f}, rs[4] = {0.f, 0.f, 0.f, 0.f};
-            int rc[4] = {0, 0, 0, 0};
+            float c4[4] = {0.f, 0.f, 0.f, 0.f}, rs[RIF];
+            int rc[RIF];
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < RIF; ++u) { rs[u] = 0.f; rc[u] = 0; }
+#pragma unroll
+            for (int u = 0; u < RIF; ++u)
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
                     if (ok[u][i]) { c4[i] += v[u][i]; ++cc[i]; rs[u] += v[u][i]; ++rc[u]; }
@@ -101,10 +104,10 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-                for (int u = 0; u < 4; ++u) { rs[u] += __shfl_xor_sync(0xffffffffu, rs[u], o); rc[u] += __shfl_xor_sync(0xffffffffu, rc[u], o); }
+                for (int u = 0; u < RIF; ++u) { rs[u] += __shfl_xor_sync(0xffffffffu, rs[u], o); rc[u] += __shfl_xor_sync(0xffffffffu, rc[u], o); }
             if (lane == 0) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
+                for (int u = 0; u < RIF; ++u)
                     if (yb + u < y1) { s_row[yb + u - y0][warp] += __float2ll_rn(rs[u] * FIX); s_cnt[yb + u - y0][warp] += rc[u]; }
             }
         }
