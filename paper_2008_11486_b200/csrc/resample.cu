@@ -47,6 +47,7 @@ constexpr int NRING = 3;      // blocks in the ring: the block being swept trail
 constexpr int WARM = 17;      // rows of forward warm-up before the first interval of a band
 constexpr int EXT = 40;       // samples beyond an image edge that are given their reflected value (the rest: 0, never used)
 constexpr size_t RESAMPLE_TWO_PASS_MAX = 64u << 20;   // stacks up to this size take the two-kernel route
+constexpr int Y4_MIN_ROWS = 32;   // shortest band of the 4-column y pass
 constexpr float U_INF = 0.26794919243112270647f;   // 2 - sqrt(3)
 
 // One axis of one frame: integer part, weights, identity flag, footprint.
@@ -84,3 +85,4 @@ __device__ __forceinline__ Axis make_axis(int n, double s)
 }  // namespace mred
 
 #include "resample_warp.cuh"
+#include "resample_ypass.cuh"

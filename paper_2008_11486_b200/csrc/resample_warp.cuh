@@ -576,10 +576,15 @@ __global__ void __launch_bounds__(32, MODE == 1 ? 16 : 8) k_resample(const float
     else warp_item<false, MODE>(it, s_ring, threadIdx.x);
 }
 
+// y pass with 4 columns per thread (resample_ypass.cuh)
+__global__ void k_ypass4(const float* __restrict__ T, int n, int w, int h, const __grid_constant__ HostShifts hs,
+                         const double* __restrict__ dshift, float fill, float* __restrict__ out, int4* __restrict__ fp_dev,
+                         int BH);
+
 // band height for the kernels that carry y state: enough warps for 148 SMs x 8, no band under 64 rows
-static int band_rows(long long cols, int h, int min_rows = 64)
+static int band_rows(long long cols, int h, int min_rows = 64, int warps_per_sm = 8)
 {
-    long long bands = (148 * 8 + cols - 1) / cols;
+    long long bands = (148 * warps_per_sm + cols - 1) / cols;
     const long long maxb = (h + min_rows - 1) / min_rows;
     if (bands > maxb) bands = maxb;
     if (bands < 1) bands = 1;
@@ -622,9 +627,15 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
         if (BH1 < 8) BH1 = 8;
         k_resample<1><<<dim3(sx1, (h + BH1 - 1) / BH1, n), 32, 0, st>>>(in, n, w, h, hs, dshift_dev, fill, tmp, nullptr, BH1, vec);
         MRED_LAUNCH_CHECK();
-        const int sx2 = (w + ModeGeom<2>::OUTC - 1) / ModeGeom<2>::OUTC;
-        const int BH2 = band_rows((long long)sx2 * n, h, 48);
-        k_resample<2><<<dim3(sx2, (h + BH2 - 1) / BH2, n), 32, smem, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2, vec);
+        if (vec) {
+            const int bx = (w + 511) / 512;
+            const int BH2 = band_rows((long long)bx * 4 * n, h, Y4_MIN_ROWS, 16);
+            k_ypass4<<<dim3(bx, (h + BH2 - 1) / BH2, n), 128, 0, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2);
+        } else {
+            const int sx2 = (w + ModeGeom<2>::OUTC - 1) / ModeGeom<2>::OUTC;
+            const int BH2 = band_rows((long long)sx2 * n, h, 48);
+            k_resample<2><<<dim3(sx2, (h + BH2 - 1) / BH2, n), 32, smem, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2, vec);
+        }
         MRED_LAUNCH_CHECK();
         return MRED_OK;
     }
