@@ -43,7 +43,8 @@ def test_host_only_calls(libpath):
     assert m.reduce_host_workspace_bytes(g, 10) >= need + 10 * 1074 * 1024 * 2
     assert m.workspace_bytes(m.CALL_COADD, g, 10) == 0
     assert m.workspace_bytes(m.CALL_RESAMPLE, g, 10) == 10 * 1024 * 1024 * 4      # small stack: two-kernel route
-    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 60) == 0                        # large stack: fused kernel
+    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 60) == 60 * 1024 * 1024 * 4
+    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 200) == 0                       # large stack: fused kernel
 
 
 def test_sass_is_sm100a(libpath):
