@@ -109,10 +109,13 @@ __device__ __forceinline__ Combined combine_mean_clip(float (&v)[NMAX], int m, b
             // running sums; the slack (1e-7 ADU at 1000 ADU) keeps them, and is far below any tie margin
             const float thr = fmaf(ksigma, sqrtf(S / (float)cnt), 1e-10f * fabsf(c));
             // cheap look first: most columns lose nothing in a pass (NaN compares false: absent entries never count)
-            bool any = false;
+            // (only for short columns: with 32+ frames some lane of the warp nearly always rejects, and the look costs a sweep)
+            if (NMAX <= 24) {
+                bool any = false;
 #pragma unroll
-            for (int i = 0; i < NMAX; ++i) any = any || (fabsf(v[i] - mean) > thr);
-            if (!any) break;
+                for (int i = 0; i < NMAX; ++i) any = any || (fabsf(v[i] - mean) > thr);
+                if (!any) break;
+            }
             float n1 = 0.f, n2 = 0.f;
             int ncnt = 0;
 #pragma unroll
