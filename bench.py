@@ -402,13 +402,30 @@ def run_ours(args):
         hplans = [mred.ReducePlan(g, n, device=devs, host=True) for _ in range(G)]
         stg = [{k: torch.empty_like(v) for k, v in d.items() if k != "sci"} for d in devg]
 
+        masters_host = [None] * G
+
         def step_host():
+            # one stream per group here too: the host->device copies of one group overlap the kernels of another
+            main = torch.cuda.current_stream()
+            fork = torch.cuda.Event()
+            fork.record(main)
             for gi in range(G):
-                for k in ("bias", "dark", "flat"):
-                    stg[gi][k].copy_(host[gi][k], non_blocking=True)
-                MB, MD, MF = mred.build_masters(g, stg[gi]["bias"], stg[gi]["dark"], groups[gi].t_dark,
-                                                stg[gi]["flat"], groups[gi].t_flat, mode=mred.MEDIAN, ws=mws)
-                mred.reduce_host(hplans[gi], host[gi]["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode)
+                st = streams[gi % len(streams)]
+                if st is not None:
+                    st.wait_event(fork)
+                with torch.cuda.stream(st) if st is not None else contextlib.nullcontext():
+                    for k in ("bias", "dark", "flat"):
+                        stg[gi][k].copy_(host[gi][k], non_blocking=True)
+                    MB, MD, MF = mred.build_masters(g, stg[gi]["bias"], stg[gi]["dark"], groups[gi].t_dark,
+                                                    stg[gi]["flat"], groups[gi].t_flat, mode=mred.MEDIAN,
+                                                    ws=mwss[gi % len(streams)], out=masters_host[gi])
+                    masters_host[gi] = (MB, MD, MF)
+                    mred.reduce_host(hplans[gi], host[gi]["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode)
+            for st in streams:
+                if st is not None:
+                    join = torch.cuda.Event()
+                    join.record(st)
+                    main.wait_event(join)
         for _ in range(2):
             step_host()
         barrier()
