@@ -18,8 +18,8 @@ constexpr float FIX = 16384.0f;    // fixed-point scale of the profile sums (2^1
 constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
 
 struct EstimateWs {
-    long long* colpart;  // [n][nbands][w]   fixed-point sums (value * FIX, see k_profiles)
-    int* colcnt;      // [n][nbands][w]
+    long long* colpart;  // [n][w]   fixed-point column sums (value * FIX), accumulated with integer atomics by the bands
+    int* colcnt;      // [n][w]   valid rows per column (contiguous after colpart: zeroed together)
     long long* rowsum;   // [n][h]
     int* rowcnt;      // [n][h]
     double* prof;     // [n][2][plen]  median-subtracted profiles (x then y)
@@ -36,8 +36,8 @@ static EstimateWs carve_est(void* ws, int w, int h, int n)
     auto take = [&](size_t b) { char* q = p; p += align_up(b, 16); return q; };
     e.nbands = (h + PROF_BR - 1) / PROF_BR;
     e.plen = w > h ? w : h;
-    e.colpart = reinterpret_cast<long long*>(take(8 * (size_t)n * e.nbands * w));
-    e.colcnt = reinterpret_cast<int*>(take(4 * (size_t)n * e.nbands * w));
+    e.colpart = reinterpret_cast<long long*>(take(8 * (size_t)n * w));
+    e.colcnt = reinterpret_cast<int*>(take(4 * (size_t)n * w));
     e.rowsum = reinterpret_cast<long long*>(take(8 * (size_t)n * h));
     e.rowcnt = reinterpret_cast<int*>(take(4 * (size_t)n * h));
     e.prof = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * e.plen));
@@ -112,8 +112,9 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
             }
         }
         for (int i = 0; i < nv; ++i) {
-            e.colpart[((size_t)k * e.nbands + band) * w + x + i] = cs[i];
-            e.colcnt[((size_t)k * e.nbands + band) * w + x + i] = cc[i];
+            // integer atomics: exact and order-independent, so no per-band partials have to be kept and re-read
+            atomicAdd(reinterpret_cast<unsigned long long*>(e.colpart) + (size_t)k * w + x + i, (unsigned long long)cs[i]);
+            atomicAdd(e.colcnt + (size_t)k * w + x + i, cc[i]);
         }
     }
     __syncthreads();
@@ -203,18 +204,8 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
             long long s = 0;
             int c = 0;
             if (axis == 0) {
-                const long long* cp = e.colpart + (size_t)k * e.nbands * w + i;
-                const int* cc = e.colcnt + (size_t)k * e.nbands * w + i;
-                int b = 0;
-                for (; b + 8 <= e.nbands; b += 8) {          // 8 bands in flight
-                    long long tv[8];
-                    int tc[8];
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) { tv[u] = __ldg(cp + (size_t)(b + u) * w); tc[u] = __ldg(cc + (size_t)(b + u) * w); }
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) { s += tv[u]; c += tc[u]; }
-                }
-                for (; b < e.nbands; ++b) { s += __ldg(cp + (size_t)b * w); c += __ldg(cc + (size_t)b * w); }
+                s = __ldg(e.colpart + (size_t)k * w + i);
+                c = __ldg(e.colcnt + (size_t)k * w + i);
             } else {
                 s = __ldg(e.rowsum + (size_t)k * h + i);
                 c = __ldg(e.rowcnt + (size_t)k * h + i);
@@ -349,6 +340,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
 {
     const EstimateWs e = carve_est(ws, w, h, n);
     const int vec_ok = (w % 4 == 0) ? 1 : 0;
+    MRED_CUDA_TRY(cudaMemsetAsync(e.colpart, 0, (size_t)(reinterpret_cast<char*>(e.colcnt) - reinterpret_cast<char*>(e.colpart)) + 4 * (size_t)n * w, st));
     k_profiles<<<dim3(e.nbands, n), 256, 0, st>>>(frames, w, h, bad, e, vec_ok);
     MRED_LAUNCH_CHECK();
     int P = 1;

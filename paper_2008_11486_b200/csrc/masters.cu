@@ -232,10 +232,24 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
     float tb = 0.f, td = 0.f;
 #pragma unroll
     for (int i = 0; i < PX; ++i) { tb += mb[i]; td += md[i]; }
-    const double sb = block_sum_256f(tb, s8);
-    const double sd = block_sum_256f(td, s8);
-    if (threadIdx.x == 0) { m.part_bd[2 * (size_t)blockIdx.x] = sb; m.part_bd[2 * (size_t)blockIdx.x + 1] = sd; }
-    if (!last_block(m.ticket)) return;
+    // block partials of both planes and the "last block" ticket with two barriers in all
+    __shared__ float2 s_w2[8];
+    __shared__ int s_lastb;
+    tb = warp_sum(tb);          // <= 64 values of one plane in float32: 1e-6 relative on a partial
+    td = warp_sum(td);
+    if ((threadIdx.x & 31) == 0) s_w2[threadIdx.x >> 5] = make_float2(tb, td);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double sb = 0.0, sd = 0.0;
+        for (int i = 0; i < 8; ++i) { sb += (double)s_w2[i].x; sd += (double)s_w2[i].y; }
+        m.part_bd[2 * (size_t)blockIdx.x] = sb;
+        m.part_bd[2 * (size_t)blockIdx.x + 1] = sd;
+        __threadfence();
+        s_lastb = (atomicAdd(m.ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_lastb) return;
+    __threadfence();
     // <G_k> = <F_k> - L_k - <MB> - r <MD>: fixed-order sums of the block partials
     double a = 0.0, b = 0.0;
     for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) { a += __ldcg(m.part_bd + 2 * (size_t)i); b += __ldcg(m.part_bd + 2 * (size_t)i + 1); }
@@ -302,9 +316,21 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
     float t = 0.f;
 #pragma unroll
     for (int i = 0; i < PX; ++i) t += mf[i];
-    const double sblk = block_sum_256f(t, s8);
-    if (threadIdx.x == 0) m.part_f[blockIdx.x] = sblk;
-    if (!last_block(m.ticket + 1)) return;
+    __shared__ float s_w1[8];
+    __shared__ int s_lastb;
+    t = warp_sum(t);
+    if ((threadIdx.x & 31) == 0) s_w1[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double sblk = 0.0;
+        for (int i = 0; i < 8; ++i) sblk += (double)s_w1[i];
+        m.part_f[blockIdx.x] = sblk;
+        __threadfence();
+        s_lastb = (atomicAdd(m.ticket + 1, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_lastb) return;
+    __threadfence();
     double a = 0.0;
     for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) a += __ldcg(m.part_f + i);
     const double sall = block_sum_256(a, s8);
