@@ -393,6 +393,60 @@ def test_config4_stress_coadd_full_size():
     _compare_coadd(st, fp, 2)
 
 
+def test_config5_geometry_two_frames():
+    """BASELINE.json config 5 geometry (4128 x 4096 raw, 4096 x 4096 image, 32 overscan columns): two frames through
+    calibrate, both resample routes and the co-add, against the oracle.  The largest frame size of the configs: 20
+    strips per row, 64 MB planes, 16-byte-aligned raw rows (8256 B)."""
+    g = synth.GEOM_LARGE
+    grp = synth.make_group(5, n_sci=2, n_master=2, stars=200)
+    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
+    MB, MD, MF = mred.build_masters(g, dev(grp.bias), dev(grp.dark), grp.t_dark, dev(grp.flat), grp.t_flat)
+    assert_close(host(MB), m.MB, "MB large")
+    assert_close(host(MF), m.MF, "MF large")
+    c = oracle.calibrate(g, grp.sci, 1.0, m.MB, m.MD, m.MF)
+    out, lev = mred.calibrate(g, dev(grp.sci), 1.0, dev(m.MB), dev(m.MD), dev(m.MF))
+    assert np.array_equal(host(lev), c.level)
+    assert_close(host(out), c.out, "calibrate large")
+    e = oracle.estimate_shifts(c.out, 0, 64)
+    ish, sh = mred.estimate_shifts(dev(c.out), 0, 64)
+    assert np.array_equal(host(ish), e.ishift) and np.max(np.abs(host(sh) - e.shift)) <= 1e-3
+    sx, sy = -e.shift[:, 0], -e.shift[:, 1]
+    r = oracle.resample(c.out[1:], sx[1:], sy[1:])
+    two, fp2 = mred.resample(dev(c.out[1:]), sx[1:], sy[1:])
+    one, fp1 = mred.resample(dev(c.out[1:]), sx[1:], sy[1:], ws=False)
+    assert np.array_equal(fp1, r.footprint) and np.array_equal(fp2, r.footprint)
+    assert_close(host(two), r.out, "resample large, two kernels", local=4)
+    assert_close(host(one), r.out, "resample large, fused", local=4)
+
+
+def test_single_frame_stacks_and_zero_lag():
+    """Degenerate sizes: one frame everywhere (a median / clipped mean of one value is that value; the only frame is
+    the reference), and max_lag = 0 (the only lag is 0, no parabola)."""
+    g = GEOMS["small"]
+    grp = synth.make_group(1, geom=g, n_sci=2, n_master=1, stars=10)
+    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
+    MB, MD, MF = mred.build_masters(g, dev(grp.bias), dev(grp.dark), grp.t_dark, dev(grp.flat), grp.t_flat)
+    assert_close(host(MB), m.MB, "MB n=1")
+    assert_close(host(MD), m.MD, "MD n=1")
+    assert_close(host(MF), m.MF, "MF n=1")
+    c = oracle.calibrate(g, grp.sci[:1], 1.0, m.MB, m.MD, m.MF)
+    out, _ = mred.calibrate(g, dev(grp.sci[:1]), 1.0, dev(m.MB), dev(m.MD), dev(m.MF))
+    assert_close(host(out), c.out, "calibrate n=1")
+    ish, sh = mred.estimate_shifts(dev(c.out), 0, 5)
+    assert np.all(host(ish) == 0) and np.all(host(sh) == 0.0)
+    c2 = oracle.calibrate(g, grp.sci, 1.0, m.MB, m.MD, m.MF)
+    e = oracle.estimate_shifts(c2.out, 1, 0)
+    ish, sh = mred.estimate_shifts(dev(c2.out), 1, 0)
+    assert np.array_equal(host(ish), e.ishift) and np.all(host(sh) == e.shift) and np.all(host(ish) == 0)
+    for mode in (0, 1, 2):
+        o, cnt, mk = mred.coadd(dev(c.out), None, mode=mode, want_mask=True)
+        assert np.array_equal(host(o), c.out[0].astype(np.float32)) and np.all(host(cnt) == 1) and np.all(host(mk) == 0)
+    r = oracle.resample(c.out, [0.37], [-1.2])
+    reg, fp = mred.resample(dev(c.out), [0.37], [-1.2])
+    assert np.array_equal(fp, r.footprint)
+    assert_close(host(reg), r.out, "resample n=1", local=4)
+
+
 # ------------------------------------------------------------------ error behaviour
 def test_error_codes():
     g = GEOMS["small"]
