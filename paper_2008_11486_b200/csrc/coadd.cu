@@ -69,11 +69,29 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
 #pragma unroll
     for (int i = 0; i < NW; ++i) m += __popc(inside[i]);
     const float* src = stack + p;
+    if (MODE != MRED_MEDIAN && NMAX <= 24 && n == NMAX && m == NMAX) {
+        // short column, every frame covers this pixel (the usual case; with 32+ frames some lane of the warp
+        // nearly always rejects something and the attempt would be wasted): unconditional loads, and a clip loop that only has to
+        // find out that nothing is rejected (bit-identical to the general path below, which takes over otherwise)
 #pragma unroll
-    for (int k = 0; k < NMAX; ++k) {
-        const bool ok = (inside[k >> 5] >> (k & 31)) & 1u;
-        v[k] = ok ? __ldcs(src) : ABSENT;
-        src += np;
+        for (int k = 0; k < NMAX; ++k) { v[k] = __ldcs(src); src += np; }
+        float value;
+        if (combine_full_noreject<NMAX>(v, MODE == MRED_SIGCLIP, ksigma, max_iter, value)) {
+            out[p] = value;
+            if (count) count[p] = (uint16_t)NMAX;
+            if (rejmask) {
+#pragma unroll
+                for (int i = 0; i < NW; ++i) rejmask[(size_t)i * np + p] = 0u;
+            }
+            return;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < NMAX; ++k) {
+            const bool ok = (inside[k >> 5] >> (k & 31)) & 1u;
+            v[k] = ok ? __ldcs(src) : ABSENT;
+            src += np;
+        }
     }
     Combined r;
     uint32_t rej[(NMAX + 31) / 32];

@@ -73,6 +73,33 @@ __device__ __forceinline__ Combined combine_median(float (&v)[NMAX], int m)
     return r;
 }
 
+// Fast path of the mean / sigma-clipped mean for a column whose NMAX entries are all present: the same float
+// operations in the same order as combine_mean_clip (so the same bits), without the absent-entry bookkeeping,
+// and v[] is left untouched.  Returns false when the first clip pass would reject something: the caller then runs
+// combine_mean_clip on the same values.
+template <int NMAX>
+__device__ __forceinline__ bool combine_full_noreject(const float (&v)[NMAX], bool clip, float ksigma, int max_iter, float& value)
+{
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < NMAX; ++i) sum += v[i];
+    const float c = sum / (float)NMAX;
+    float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int i = 0; i < NMAX; ++i) { const float d = v[i] - c; s1 += d; s2 = fmaf(d, d, s2); }
+    const float mean = s1 / (float)NMAX;
+    if (clip && max_iter > 0) {
+        const float S = fmaxf(s2 - mean * s1, 0.f);
+        const float thr = fmaf(ksigma, sqrtf(S / (float)NMAX), 1e-10f * fabsf(c));
+        bool any = false;
+#pragma unroll
+        for (int i = 0; i < NMAX; ++i) any = any || (fabsf((v[i] - c) - mean) > thr);
+        if (any) return false;
+    }
+    value = c + mean;
+    return true;
+}
+
 // Mean / sigma-clipped mean.  On entry absent entries hold NaN and `m` counts the valid ones;
 // on exit every entry that was not used holds NaN (so the caller can build the rejection mask).
 //   c      = sum(v)/m                       (float32 approximation of the mean)
