@@ -388,9 +388,12 @@ def run_ours(args):
             "resample": "k_resample<1> + k_ypass4 (x pass, y pass)" if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else "k_resample<0>",
             "coadd": "k_coadd"}[dom]
     traffic = None
-    tr_path = os.path.join(ROOT, "profiles", "traffic.json")      # ncu --set full capture of config 2 (profiles/r1f_kernels.md)
+    tr_path = os.path.join(ROOT, "profiles", "traffic.csv")       # DRAM bytes per launch from the ncu --set full captures of config 2
     if cfg == 2 and os.path.exists(tr_path):
-        traffic = json.load(open(tr_path)).get(dom)
+        for line in open(tr_path).read().splitlines()[1:]:
+            parts = line.split(",")
+            if parts and parts[0] == dom:
+                traffic = int(parts[1])
     roof = {"bound": "hbm", "kernel": kern, "stage": dom, "achieved": ref_stages[dom]["GBps"], "peak": peak,
             "peak_source": peak_src, "unit": "GB/s", "frac": ref_stages[dom]["frac"], "traffic": traffic,
             "algorithmic_bytes_per_launch": sb[dom], "launch_ms": ref_stages[dom]["ms_per_call"],
