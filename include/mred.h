@@ -119,7 +119,7 @@ int mred_estimate_shifts(const float *frames, int n, int w, int h, int ref_index
  * in/out: float32 [n][h][w] (must not overlap); sx, sy: HOST float64 [n];
  * footprint: HOST int32 [n][4] output {x_lo, x_hi, y_lo, y_hi} inclusive (nullable) --
  * written before the call returns.  w, h >= 4.  ws is optional: with at least
- * mred_workspace_bytes(MRED_CALL_RESAMPLE, ..) bytes (non-zero only for stacks up to 512 MB) the
+ * mred_workspace_bytes(MRED_CALL_RESAMPLE, ..) bytes (non-zero only for planes up to 16 MB and stacks up to 4 GB) the
  * shift runs as an x kernel and a y kernel with the intermediate held in ws; without it, as one fused kernel.
  * Both routes give the same result to float32 rounding.
  */

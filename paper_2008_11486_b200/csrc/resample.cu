@@ -46,7 +46,8 @@ constexpr int RB = 8;         // rows per block of the y pass
 constexpr int NRING = 3;      // blocks in the ring: the block being swept trails the loads by 16 rows
 constexpr int WARM = 17;      // rows of forward warm-up before the first interval of a band
 constexpr int EXT = 40;       // samples beyond an image edge that are given their reflected value (the rest: 0, never used)
-constexpr size_t RESAMPLE_TWO_PASS_MAX = (size_t)512 << 20;   // stacks up to this size take the two-kernel route (measured: faster up to 60 x 1024^2; 100 x 4096^2 is faster fused)
+constexpr size_t RESAMPLE_TWO_PASS_MAX = (size_t)4 << 30;        // two-kernel route: stacks up to this size ...
+constexpr size_t RESAMPLE_TWO_PASS_PLANE = (size_t)16 << 20;     // ... of planes up to this size (measured: 200 x 1024^2 0.83 ms in two kernels; 100 x 4096^2 5.4 ms fused, 6.5 ms in two)
 constexpr int Y4_MIN_ROWS = 32;   // shortest band of the 4-column y pass
 constexpr float U_INF = 0.26794919243112270647f;   // 2 - sqrt(3)
 

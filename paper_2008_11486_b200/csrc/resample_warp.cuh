@@ -594,8 +594,8 @@ static int band_rows(long long cols, int h, int min_rows = 64, int warps_per_sm 
 
 size_t resample_ws_bytes(int w, int h, int n)
 {
-    const size_t b = (size_t)n * w * h * sizeof(float);
-    return b <= RESAMPLE_TWO_PASS_MAX ? b : 0;
+    const size_t plane = (size_t)w * h * sizeof(float), b = plane * (size_t)n;
+    return (b <= RESAMPLE_TWO_PASS_MAX && plane <= RESAMPLE_TWO_PASS_PLANE) ? b : 0;
 }
 
 int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,

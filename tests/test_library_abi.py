@@ -44,7 +44,7 @@ def test_host_only_calls(libpath):
     assert m.workspace_bytes(m.CALL_COADD, g, 10) == 0
     assert m.workspace_bytes(m.CALL_RESAMPLE, g, 10) == 10 * 1024 * 1024 * 4      # small stack: two-kernel route
     assert m.workspace_bytes(m.CALL_RESAMPLE, g, 60) == 60 * 1024 * 1024 * 4
-    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 200) == 0                       # large stack: fused kernel
+    assert m.workspace_bytes(m.CALL_RESAMPLE, (4128, 4096, 0, 32, 32, 0, 4096, 4096), 100) == 0   # large planes: fused kernel
 
 
 def test_sass_is_sm100a(libpath):
