@@ -35,7 +35,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
-        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= newest:
+        # an object is stale when its own .cu, any shared header (.cuh) or mred.h is newer
+        hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if not f.endswith(".cu")]
+        hdrs += [os.path.join(HERE, "..", "include", "mred.h"), os.path.join(CSRC, src)]
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(f) for f in hdrs):
             return obj
         cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)

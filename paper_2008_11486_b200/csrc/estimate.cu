@@ -4,7 +4,8 @@
 //
 //   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): fixed-point (int64) column
 //                partial sums per 32-row band and complete row sums, valid-pixel counts.
-//   k_finalize : per (frame, axis): fixed-order band sum, mean, median by a shared-memory radix select, subtract.
+//   k_finalize : per (frame, axis): mean from the integer sums, median by a bitonic sort (registers + shuffles inside
+//                a warp, shared memory across warps), subtract.
 //   k_correlate: per (frame, axis): C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
 //                smaller |l| then smaller l; 3-point parabola.
 // No float atomics: every sum has a fixed order, so the integer result is reproducible.
@@ -19,12 +20,12 @@ constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds 
 
 struct EstimateWs {
     long long* colpart;  // [n][w]   fixed-point column sums (value * FIX), accumulated with integer atomics by the bands
-    int* colcnt;      // [n][w]   valid rows per column (contiguous after colpart: zeroed together)
+    int* colcnt;      // [n][w]   valid rows per column (contiguous after colpart: zeroed together; used with a mask only)
+    unsigned int* ticket;  // [n][2] block counters of k_correlate (contiguous after colcnt: zeroed by the same memset)
     long long* rowsum;   // [n][h]
     int* rowcnt;      // [n][h]
     double* prof;     // [n][2][plen]  median-subtracted profiles (x then y)
     double* corr;     // [n][2][2*MRED_MAX_LAG+1]  C(l) of every lag
-    unsigned int* ticket;  // [n][2] block counters of k_correlate (zeroed per call)
     size_t bytes;
     int nbands, plen;
 };
@@ -38,11 +39,11 @@ static EstimateWs carve_est(void* ws, int w, int h, int n)
     e.plen = w > h ? w : h;
     e.colpart = reinterpret_cast<long long*>(take(8 * (size_t)n * w));
     e.colcnt = reinterpret_cast<int*>(take(4 * (size_t)n * w));
+    e.ticket = reinterpret_cast<unsigned int*>(take(4 * (size_t)n * 2));
     e.rowsum = reinterpret_cast<long long*>(take(8 * (size_t)n * h));
     e.rowcnt = reinterpret_cast<int*>(take(4 * (size_t)n * h));
     e.prof = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * e.plen));
     e.corr = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * (2 * MRED_MAX_LAG + 1)));
-    e.ticket = reinterpret_cast<unsigned int*>(take(4 * (size_t)n * 2));
     e.bytes = (size_t)(p - static_cast<char*>(ws));
     return e;
 }
@@ -114,7 +115,7 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
         for (int i = 0; i < nv; ++i) {
             // integer atomics: exact and order-independent, so no per-band partials have to be kept and re-read
             atomicAdd(reinterpret_cast<unsigned long long*>(e.colpart) + (size_t)k * w + x + i, (unsigned long long)cs[i]);
-            atomicAdd(e.colcnt + (size_t)k * w + x + i, cc[i]);
+            if (bad) atomicAdd(e.colcnt + (size_t)k * w + x + i, cc[i]);
         }
     }
     __syncthreads();
@@ -123,7 +124,7 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
         int c = 0;
         for (int i = 0; i < 8; ++i) { t += s_row[r][i]; c += s_cnt[r][i]; }
         e.rowsum[(size_t)k * h + y0 + r] = t;
-        e.rowcnt[(size_t)k * h + y0 + r] = c;
+        if (bad) e.rowcnt[(size_t)k * h + y0 + r] = c;
     }
 }
 
@@ -139,60 +140,52 @@ __device__ __forceinline__ double val_of(unsigned long long k)
     return __longlong_as_double((long long)u);
 }
 
-struct SelectScratch { unsigned int hist[256]; unsigned long long prefix; unsigned int rank; unsigned long long red[32]; };
-
-// key of rank r (0-based, ascending) among keys[0..P): 8-bit radix select, 8 passes (block-wide call)
-__device__ unsigned long long block_select(const unsigned long long* keys, int P, unsigned int r, SelectScratch* sc)
+// Ascending bitonic sort of keys[0..P) in shared memory, P a power of two (block-wide call, blockDim.x = 1024).
+// P <= 1024: one key per thread in a register; the 40 of 55 exchange steps whose partner sits in the same warp are two
+// shuffles, only the 15 cross-warp steps go through shared memory (two barriers each).  Larger P: pairs in shared memory.
+// A data-independent ~3 us, where the 8-pass radix select it replaces spent ~20 us in barriers and same-bin atomics.
+__device__ void block_sort(unsigned long long* keys, int P)
 {
-    if (threadIdx.x == 0) { sc->prefix = 0ULL; sc->rank = r; }
-    unsigned long long mask = 0ULL;
-    for (int shift = 56; shift >= 0; shift -= 8) {
-        for (int i = threadIdx.x; i < 256; i += blockDim.x) sc->hist[i] = 0u;
-        __syncthreads();
-        const unsigned long long prefix = sc->prefix;
-        for (int i = threadIdx.x; i < P; i += blockDim.x) {
-            // profile values share their leading bytes, so in the first passes a whole warp hits ONE bin: count such a
-            // warp with a single atomic (vote, not __match_any_sync: MATCH costs hundreds of cycles per call here)
-            const unsigned long long k = keys[i];
-            const unsigned int am = __activemask();
-            const unsigned int d = ((k & mask) == prefix) ? ((unsigned int)(k >> shift) & 255u) : 256u;
-            const int leader = __ffs(am) - 1;
-            const unsigned int d0 = __shfl_sync(am, d, leader);
-            if (__all_sync(am, d == d0)) {
-                if ((int)(threadIdx.x & 31) == leader && d < 256u) atomicAdd(&sc->hist[d], (unsigned int)__popc(am));
-            } else if (d < 256u) {
-                atomicAdd(&sc->hist[d], 1u);
-            }
-        }
-        __syncthreads();
-        if (threadIdx.x < 32) {          // warp 0: find the bin that holds the rank (8 bins per lane)
-            const int lane = threadIdx.x;
-            unsigned int loc[8], tot = 0;
-#pragma unroll
-            for (int u = 0; u < 8; ++u) { loc[u] = sc->hist[8 * lane + u]; tot += loc[u]; }
-            unsigned int inc = tot;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-            const unsigned int before = inc - tot, rk = sc->rank;
-            if (rk >= before && rk < inc) {          // exactly one lane
-                unsigned int cum = before;
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    if (rk >= cum && rk < cum + loc[u]) { sc->prefix = prefix | ((unsigned long long)(8 * lane + u) << shift); sc->rank = rk - cum; }
-                    cum += loc[u];
+    if (P <= (int)blockDim.x) {
+        const int i = threadIdx.x;
+        unsigned long long v = i < P ? keys[i] : ~0ULL;
+        for (int k = 2; k <= P; k <<= 1) {
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                unsigned long long o;
+                if (j >= 32) {
+                    __syncthreads();
+                    if (i < P) keys[i] = v;
+                    __syncthreads();
+                    o = i < P ? keys[i ^ j] : v;
+                } else {
+                    o = __shfl_xor_sync(0xffffffffu, v, j);
                 }
+                const bool takemin = (((i & j) == 0) == ((i & k) == 0));
+                v = takemin ? (o < v ? o : v) : (o > v ? o : v);
             }
         }
-        mask |= 255ULL << shift;
         __syncthreads();
+        if (i < P) keys[i] = v;
+        __syncthreads();
+        return;
     }
-    return sc->prefix;
+    for (int k = 2; k <= P; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            __syncthreads();
+            for (int t = threadIdx.x; t < (P >> 1); t += blockDim.x) {
+                const int i = 2 * t - (t & (j - 1)), l = i + j;
+                const unsigned long long a = keys[i], b = keys[l];
+                if ((a > b) == ((i & k) == 0)) { keys[i] = b; keys[l] = a; }
+            }
+        }
+    }
+    __syncthreads();
 }
 
 // Median-subtracted mean profile of frame k along `axis` into dst[0..len) (shared memory); keys[0..P) is scratch
-// for the selection (invalid lines get the +inf key, which sorts last).  All threads of the block call it.
-__device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis, int len, int P, double* dst,
-                              unsigned long long* keys, SelectScratch* sc, int* s_m)
+// for the sort (invalid lines get the +inf key, which sorts last).  All threads of the block call it.
+__device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis, int len, int P, int has_bad,
+                              double* dst, unsigned long long* keys, int* s_m)
 {
     const double INF = __longlong_as_double(0x7ff0000000000000LL);
     if (threadIdx.x == 0) *s_m = 0;
@@ -202,13 +195,13 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
         double v = INF;
         if (i < len) {
             long long s = 0;
-            int c = 0;
+            int c = axis == 0 ? h : w;         // without a bad-pixel mask every line is complete
             if (axis == 0) {
-                s = __ldg(e.colpart + (size_t)k * w + i);
-                c = __ldg(e.colcnt + (size_t)k * w + i);
+                s = __ldcg(e.colpart + (size_t)k * w + i);
+                if (has_bad) c = __ldcg(e.colcnt + (size_t)k * w + i);
             } else {
-                s = __ldg(e.rowsum + (size_t)k * h + i);
-                c = __ldg(e.rowcnt + (size_t)k * h + i);
+                s = __ldcg(e.rowsum + (size_t)k * h + i);
+                if (has_bad) c = __ldcg(e.rowcnt + (size_t)k * h + i);
             }
             if (c > 0) { v = (double)s / ((double)FIX * (double)c); ++mine; }
             dst[i] = v;
@@ -221,33 +214,9 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
     const int m = *s_m;
     double med = 0.0;
     if (m > 0) {
-        const unsigned long long ka = block_select(keys, P, (unsigned int)((m - 1) >> 1), sc);
-        med = val_of(ka);
-        if (!(m & 1)) {
-            // rank m/2 = next order statistic: ka again if it is repeated often enough, else the smallest key above it
-            unsigned int le = 0;
-            unsigned long long mn = ~0ULL;
-            for (int i = threadIdx.x; i < P; i += blockDim.x) {
-                const unsigned long long kk = keys[i];
-                le += kk <= ka;
-                if (kk > ka && kk < mn) mn = kk;
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                le += __shfl_xor_sync(0xffffffffu, le, o);
-                const unsigned long long t = __shfl_xor_sync(0xffffffffu, mn, o);
-                mn = t < mn ? t : mn;
-            }
-            __syncthreads();
-            if ((threadIdx.x & 31) == 0) { sc->red[threadIdx.x >> 5] = mn; sc->hist[threadIdx.x >> 5] = le; }
-            __syncthreads();
-            unsigned int le_all = 0;
-            unsigned long long mn_all = ~0ULL;
-            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { le_all += sc->hist[i]; mn_all = sc->red[i] < mn_all ? sc->red[i] : mn_all; }
-            const double b = (le_all > (unsigned int)(m >> 1)) ? med : val_of(mn_all);
-            med = 0.5 * (med + b);
-            __syncthreads();
-        }
+        block_sort(keys, P);
+        med = val_of(keys[(m - 1) >> 1]);
+        if (!(m & 1)) med = 0.5 * (med + val_of(keys[m >> 1]));
     }
     for (int i = threadIdx.x; i < len; i += blockDim.x) {
         const double v = dst[i];
@@ -257,10 +226,9 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
 }
 
 // grid (n, 2), block 1024: median-subtracted mean profile of (frame, axis) -> e.prof
-__global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
+__global__ void __launch_bounds__(1024) k_finalize(int w, int h, int has_bad, EstimateWs e)
 {
-    extern __shared__ double s_dyn[];     // profile[P], selection keys[P]
-    __shared__ SelectScratch s_sc;
+    extern __shared__ double s_dyn[];     // profile[P], sort keys[P]
     __shared__ int s_m;
     const int k = blockIdx.x, axis = blockIdx.y;
     const int len = axis == 0 ? w : h;
@@ -268,7 +236,7 @@ __global__ void __launch_bounds__(1024) k_finalize(int w, int h, EstimateWs e)
     while (P < len) P <<= 1;
     double* a = s_dyn;
     unsigned long long* keys = reinterpret_cast<unsigned long long*>(s_dyn + P);
-    block_profile(e, w, h, k, axis, len, P, a, keys, &s_sc, &s_m);
+    block_profile(e, w, h, k, axis, len, P, has_bad, a, keys, &s_m);
     double* out = e.prof + ((size_t)k * 2 + axis) * e.plen;
     for (int i = threadIdx.x; i < len; i += blockDim.x) out[i] = a[i];
 }
@@ -340,7 +308,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
 {
     const EstimateWs e = carve_est(ws, w, h, n);
     const int vec_ok = (w % 4 == 0) ? 1 : 0;
-    MRED_CUDA_TRY(cudaMemsetAsync(e.colpart, 0, (size_t)(reinterpret_cast<char*>(e.colcnt) - reinterpret_cast<char*>(e.colpart)) + 4 * (size_t)n * w, st));
+    MRED_CUDA_TRY(cudaMemsetAsync(e.colpart, 0, (size_t)(reinterpret_cast<char*>(e.ticket) - reinterpret_cast<char*>(e.colpart)) + 4 * (size_t)n * 2, st));
     k_profiles<<<dim3(e.nbands, n), 256, 0, st>>>(frames, w, h, bad, e, vec_ok);
     MRED_LAUNCH_CHECK();
     int P = 1;
@@ -351,9 +319,8 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_correlate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
         attr_done = true;
     }
-    k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, e);
+    k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, bad ? 1 : 0, e);
     MRED_LAUNCH_CHECK();
-    MRED_CUDA_TRY(cudaMemsetAsync(e.ticket, 0, sizeof(unsigned int) * 2 * (size_t)n, st));
     k_correlate<<<dim3(n, 2, CORR_Z), 256, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;

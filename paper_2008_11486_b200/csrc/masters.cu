@@ -170,7 +170,9 @@ __device__ __forceinline__ bool last_block(unsigned int* ticket)
 }
 
 // ---- bias + dark; the last block turns the block sums into 1/<G_k> of every flat ----------------
-template <int NMAX, int MODE, int PX>
+// FULL: both stacks hold exactly NMAX frames (the usual case), so every "k < n" test below is a compile-time
+// constant: no predicates, no absent-entry selects (a quarter of the instructions of this issue-bound kernel)
+template <int NMAX, int MODE, int PX, bool FULL>
 __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__ bias, int nb,
                                                     const uint16_t* __restrict__ dark, int nd, int nf, Geom g,
                                                     MastersWs m, double r, float ksigma, int max_iter,
@@ -204,21 +206,21 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
             float o[PX], od[PX];
 #pragma unroll
             for (int i = 0; i < PX; ++i) { o[i] = 0.f; od[i] = 0.f; }
-            if (k < nb) load_px<PX>(pb, 0, nv, o);
-            if (k < nd) load_px<PX>(pd, 0, nv, od);
+            if (FULL || k < nb) load_px<PX>(pb, 0, nv, o);
+            if (FULL || k < nd) load_px<PX>(pd, 0, nv, od);
             pb += fs; pd += fs;
 #pragma unroll
-            for (int i = 0; i < PX; ++i) { v[i][k] = k < nb ? o[i] - s_lb[k] : ABSENT; dk[i][k] = od[i]; }
+            for (int i = 0; i < PX; ++i) { v[i][k] = (FULL || k < nb) ? o[i] - s_lb[k] : ABSENT; dk[i][k] = od[i]; }
         }
 #pragma unroll
-        for (int i = 0; i < PX; ++i) mb[i] = combine_all<NMAX, MODE>(v[i], nb, ksigma, max_iter);
+        for (int i = 0; i < PX; ++i) mb[i] = combine_all<NMAX, MODE>(v[i], FULL ? NMAX : nb, ksigma, max_iter);
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
 #pragma unroll
-            for (int i = 0; i < PX; ++i) v[i][k] = k < nd ? (dk[i][k] - s_ld[k]) - mb[i] : ABSENT;
+            for (int i = 0; i < PX; ++i) v[i][k] = (FULL || k < nd) ? (dk[i][k] - s_ld[k]) - mb[i] : ABSENT;
         }
 #pragma unroll
-        for (int i = 0; i < PX; ++i) md[i] = combine_all<NMAX, MODE>(v[i], nd, ksigma, max_iter);
+        for (int i = 0; i < PX; ++i) md[i] = combine_all<NMAX, MODE>(v[i], FULL ? NMAX : nd, ksigma, max_iter);
         if (PX == 2) {
             *reinterpret_cast<float2*>(MB + p) = make_float2(mb[0], mb[PX - 1]);
             *reinterpret_cast<float2*>(MD + p) = make_float2(md[0], md[PX - 1]);
@@ -266,7 +268,7 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
 }
 
 // ---- flat; the last block turns the block sums into 1/<MF_raw> ---------------------------------
-template <int NMAX, int MODE, int PX>
+template <int NMAX, int MODE, int PX, bool FULL>
 __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ flat, int nb, int nd, int nf, Geom g,
                                                    MastersWs m, float r, float ksigma, int max_iter,
                                                    const float* __restrict__ MB, const float* __restrict__ MD,
@@ -300,13 +302,13 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX];
-            if (k < nf) load_px<PX>(pf, 0, nv, o);
+            if (FULL || k < nf) load_px<PX>(pf, 0, nv, o);
             pf += fs;
 #pragma unroll
-            for (int i = 0; i < PX; ++i) v[i][k] = k < nf ? ((o[i] - s_lf[k]) - off[i]) * s_ig[k] : ABSENT;
+            for (int i = 0; i < PX; ++i) v[i][k] = (FULL || k < nf) ? ((o[i] - s_lf[k]) - off[i]) * s_ig[k] : ABSENT;
         }
 #pragma unroll
-        for (int i = 0; i < PX; ++i) mf[i] = combine_all<NMAX, MODE>(v[i], nf, ksigma, max_iter);
+        for (int i = 0; i < PX; ++i) mf[i] = combine_all<NMAX, MODE>(v[i], FULL ? NMAX : nf, ksigma, max_iter);
         if (PX == 2) *reinterpret_cast<float2*>(MF + p) = make_float2(mf[0], mf[PX - 1]);
         else for (int i = 0; i < nv; ++i) MF[p + i] = mf[i];
 #pragma unroll
@@ -352,28 +354,28 @@ __global__ void __launch_bounds__(256) k_mf_scale(float* __restrict__ MF, size_t
     }
 }
 
-template <int NMAX, int PX>
+template <int NMAX, int PX, bool FULL>
 static void launch_bd(int mode, dim3 grid, cudaStream_t st, const uint16_t* bias, int nb, const uint16_t* dark, int nd,
                       int nf, const Geom& g, const MastersWs& m, double r, float ks, int mi, float* MB, float* MD)
 {
     if (mode == MRED_MEDIAN)
-        k_masters_bd<NMAX, MRED_MEDIAN, PX><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
+        k_masters_bd<NMAX, MRED_MEDIAN, PX, FULL><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
     else if (mode == MRED_MEAN)
-        k_masters_bd<NMAX, MRED_MEAN, PX><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
+        k_masters_bd<NMAX, MRED_MEAN, PX, FULL><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
     else
-        k_masters_bd<NMAX, MRED_SIGCLIP, PX><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
+        k_masters_bd<NMAX, MRED_SIGCLIP, PX, FULL><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
 }
 
-template <int NMAX, int PX>
+template <int NMAX, int PX, bool FULL>
 static void launch_f(int mode, dim3 grid, cudaStream_t st, const uint16_t* flat, int nb, int nd, int nf, const Geom& g,
                      const MastersWs& m, float r, float ks, int mi, const float* MB, const float* MD, float* MF)
 {
     if (mode == MRED_MEDIAN)
-        k_masters_f<NMAX, MRED_MEDIAN, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
+        k_masters_f<NMAX, MRED_MEDIAN, PX, FULL><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
     else if (mode == MRED_MEAN)
-        k_masters_f<NMAX, MRED_MEAN, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
+        k_masters_f<NMAX, MRED_MEAN, PX, FULL><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
     else
-        k_masters_f<NMAX, MRED_SIGCLIP, PX><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
+        k_masters_f<NMAX, MRED_SIGCLIP, PX, FULL><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
 }
 
 // capacity buckets (the sorting network and every sweep are unrolled over the capacity, so a tight bucket
@@ -414,16 +416,18 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     const double rd = (double)t_flat / (double)t_dark;
 #define CALL_BD(N, PX)                                                                                         \
     do {                                                                                                       \
-        if (PX == 2 && pair_ok) launch_bd<N, PX>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
-        else launch_bd<N, 1>(o.mode, dim3((unsigned)((np + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        if (PX == 2 && pair_ok && nb == N && nd == N) launch_bd<N, PX, true>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        else if (PX == 2 && pair_ok) launch_bd<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        else launch_bd<N, 1, false>(o.mode, dim3((unsigned)((np + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
     } while (0)
     MRED_BUCKET(nbd, CALL_BD);
 #undef CALL_BD
     MRED_LAUNCH_CHECK();
 #define CALL_F(N, PX)                                                                                          \
     do {                                                                                                       \
-        if (PX == 2 && pair_ok) launch_f<N, PX>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
-        else launch_f<N, 1>(o.mode, dim3((unsigned)((np + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        if (PX == 2 && pair_ok && nf == N) launch_f<N, PX, true>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        else if (PX == 2 && pair_ok) launch_f<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        else launch_f<N, 1, false>(o.mode, dim3((unsigned)((np + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
     } while (0)
     MRED_BUCKET(nf, CALL_F);
 #undef CALL_F
