@@ -75,13 +75,15 @@ def max_over_ranks(value, device=None):
     return float(t.item())
 
 
-def stage_bytes(g, n, nm, want_mask_words=0):
-    """Algorithmic bytes per call (every input byte read once, every output byte written once); DESIGN.md."""
+def stage_bytes(g, n, nm, want_mask_words=0, fused_profiles=False):
+    """Algorithmic bytes per call (every input byte read once, every output byte written once); DESIGN.md.
+    fused_profiles: the chained path without a bad-pixel mask sums the marginal profiles inside the calibrate kernel,
+    so estimate_shifts reads only those sums ("0 if fused into calibrate")."""
     raw, img = 2 * g.W * g.H, 4 * g.w * g.h
     return {
         "build_masters": 3 * nm * raw + 3 * img,
         "calibrate": n * (raw + img) + 3 * img,
-        "estimate_shifts": n * img,
+        "estimate_shifts": n * 8 * (g.w + g.h) if fused_profiles else n * img,
         "resample": 2 * n * img,
         "coadd": n * img + img + img // 2 + want_mask_words * img,
     }
@@ -206,6 +208,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 KERNELS_PER_BUILD_MASTERS = 4    # k_master_sums, k_masters_bd, k_masters_f, k_mf_scale
 KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd (+1: small stacks resample in two kernels); memset nodes not counted
+KERNELS_PER_REDUCE_FUSED = 6     # without a bad-pixel mask k_calibrate_prof replaces k_calibrate + k_profiles
 
 
 def run_ours(args):
@@ -337,7 +340,8 @@ def run_ours(args):
     value = frames_per_step * args.steps / (total_ms * 1e-3)
 
     # per-stage device times inside the timed region (average per call = per group)
-    sb = stage_bytes(g, n, nm, words)
+    fused = all(b is None for b in bad)
+    sb = stage_bytes(g, n, nm, words, fused_profiles=fused)
     st_ms = {k: [] for k in ["build_masters"] + STAGES}
     for evm, evs in stage_ev:
         for gi in range(G):
@@ -384,7 +388,8 @@ def run_ours(args):
     # on several streams (an event interval on one stream then also holds the other streams' kernels)
     ref_stages = stages_iso if stages_iso is not None else stages
     dom = max(STAGES, key=lambda k: ref_stages[k]["ms_per_call"])
-    kern = {"calibrate": "k_calibrate (+k_frame_sums)", "estimate_shifts": "k_profiles (+k_finalize, k_correlate)",
+    kern = {"calibrate": ("k_calibrate_prof" if fused else "k_calibrate") + " (+k_frame_sums)",
+            "estimate_shifts": "k_finalize, k_correlate (profile sums come from k_calibrate_prof)" if fused else "k_profiles (+k_finalize, k_correlate)",
             "resample": "k_resample<1> + k_ypass4 (x pass, y pass)" if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else "k_resample<0>",
             "coadd": "k_coadd"}[dom]
     traffic = None
@@ -478,7 +483,7 @@ def run_ours(args):
                            "coadd": ["median", "mean", "sigclip 3.0 x3"][mode], "l2": "512 MB flush before every step",
                            "parallelism": "groups sharded over ranks, no collective", "streams": len(streams), "launch": "cuda graph replay" if graph is not None else "plain launches",
                            "stage_timing": "CUDA events inside the C call; with a graph: instrumented plain-launch passes of the same step right after the timed region"},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + KERNELS_PER_REDUCE + (1 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 0)),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + (KERNELS_PER_REDUCE_FUSED if fused else KERNELS_PER_REDUCE) + (1 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 0)),
                 "roofline": roof, "stages": stages, "stages_isolated": stages_iso, "path_roofline": e2e_roof, "cpu_baseline": cpu,
                 "wall_s_timed_region": round(wall, 4), "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU "
                 "stages on a TITAN X (Pascal) = ~870 frames/s (other hardware, other data; context only)"}

@@ -21,7 +21,7 @@ static bool opts_ok(const mred_comb_opts* o)
 struct ReduceWs {
     float* cal;               // [n][h][w]
     float* reg;               // [n][h][w]
-    unsigned long long* os;   // [n]
+    unsigned long long* os;   // [n][frame_sums_parts] block partials of the overscan sums
     int32_t* ishift;          // [n][2]
     double* shift;            // [n][2]
     int32_t* fp;              // [n][4]
@@ -39,7 +39,7 @@ static ReduceWs carve_reduce(void* ws, const Geom& g, int n)
     const size_t np = (size_t)g.w * g.h;
     r.cal = reinterpret_cast<float*>(take(4 * np * n));
     r.reg = reinterpret_cast<float*>(take(4 * np * n));
-    r.os = reinterpret_cast<unsigned long long*>(take(8 * (size_t)n));
+    r.os = reinterpret_cast<unsigned long long*>(take(8 * (size_t)n * frame_sums_parts(g)));
     r.ishift = reinterpret_cast<int32_t*>(take(8 * (size_t)n));
     r.shift = reinterpret_cast<double*>(take(16 * (size_t)n));
     r.fp = reinterpret_cast<int32_t*>(take(16 * (size_t)n));
@@ -101,7 +101,7 @@ size_t mred_workspace_bytes(int call, const mred_geom* geom, int n)
     const Geom g = to_geom(geom);
     switch (call) {
         case MRED_CALL_BUILD_MASTERS: return masters_ws_bytes(g, n);
-        case MRED_CALL_CALIBRATE: return align_up(8 * (size_t)n, 16);
+        case MRED_CALL_CALIBRATE: return align_up(8 * (size_t)n * frame_sums_parts(g), 16);
         case MRED_CALL_ESTIMATE_SHIFTS: return estimate_ws_bytes(g.w, g.h, n);
         case MRED_CALL_RESAMPLE: return resample_ws_bytes(g.w, g.h, n);   /* optional: without it the one-kernel route runs */
         case MRED_CALL_COADD: return 0;
@@ -139,13 +139,13 @@ int mred_calibrate(const mred_geom* geom, const uint16_t* raw, int n, float dark
 {
     if (!geom_ok(geom) || !raw || !MB || !MD || !MF || !out || n < 1 || n > 65535 * 8) return MRED_EINVAL;
     if (!aligned16(raw) || !aligned16(MB) || !aligned16(MD) || !aligned16(MF) || !aligned16(out)) return MRED_EALIGN;
-    if (!ws || !aligned16(ws) || ws_bytes < 8 * (size_t)n) return MRED_EWORKSPACE;
     const Geom g = to_geom(geom);
+    if (!ws || !aligned16(ws) || ws_bytes < 8 * (size_t)n * frame_sums_parts(g)) return MRED_EWORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     unsigned long long* os = static_cast<unsigned long long*>(ws);
-    int rc = launch_frame_sums(raw, g, n, os, nullptr, st);
+    int rc = launch_frame_sums(raw, g, n, os, nullptr, 0, st);
     if (rc) return rc;
-    return launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, out, level_out, os, nullptr, st);
+    return launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, out, level_out, os, st);
 }
 
 int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index, int max_lag,
@@ -159,7 +159,7 @@ int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index
     if (!aligned16(frames) || !aligned16(ishift) || !aligned16(shift) || (badmask && !aligned16(badmask)))
         return MRED_EALIGN;
     if (!ws || !aligned16(ws) || ws_bytes < estimate_ws_bytes(w, h, n)) return MRED_EWORKSPACE;
-    return launch_estimate(frames, n, w, h, ref_index, max_lag, badmask, ishift, shift, ws,
+    return launch_estimate(frames, n, w, h, ref_index, max_lag, badmask, ishift, shift, ws, 0,
                            static_cast<cudaStream_t>(stream));
 }
 
@@ -214,12 +214,25 @@ int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float 
 #define MRED_STAGE_EVENT(i) \
     do { if (events && events[i]) MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[i]), st)); } while (0)
     MRED_STAGE_EVENT(0);
-    if ((rc = launch_frame_sums(raw, g, n, r.os, nullptr, st))) return rc;
-    if ((rc = launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, r.cal, nullptr, r.os, nullptr, st))) return rc;
+    // The level kernel also clears the accumulators of estimate_shifts (no memset node between the stages); without
+    // a bad-pixel mask the calibrate kernel sums the marginal profiles itself, so estimate_shifts starts at its
+    // finalize kernel and the calibrated stack is not re-read.
+    void* zero;
+    size_t zero_bytes;
+    long long *colsum, *rowsum;
+    estimate_accumulators(r.est, g.w, g.h, n, &zero, &zero_bytes, &colsum, &rowsum);
+    if ((rc = launch_frame_sums(raw, g, n, r.os, zero, zero_bytes, st))) return rc;
+    int est_flags = EST_ZEROED;
+    if (!badmask) {
+        if ((rc = launch_calibrate_prof(raw, g, n, dark_scale, MB, MD, MF, r.cal, r.os, colsum, rowsum, st))) return rc;
+        est_flags |= EST_HAVE_SUMS;
+    } else {
+        if ((rc = launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, r.cal, nullptr, r.os, st))) return rc;
+    }
     MRED_STAGE_EVENT(1);
     double* shift = shift_out ? shift_out : r.shift;
     int32_t* fp = footprint_out ? footprint_out : r.fp;
-    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, st))) return rc;
+    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, est_flags, st))) return rc;
     MRED_STAGE_EVENT(2);
     if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, r.rs, r.rs_bytes, st))) return rc;
     MRED_STAGE_EVENT(3);

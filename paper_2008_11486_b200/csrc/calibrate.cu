@@ -9,31 +9,55 @@
 namespace mred {
 
 // ---------------------------------------------------------------------------------------------
-// Exact integer sums: overscan columns of every frame, optionally the image rectangle as well
-// (used for <F_k> of the flats).  Integer atomics -> order-independent, bit-exact.
-// grid (row_chunks, n), block 256; each warp takes rows r0 + warp, r0 + warp + 8, ...
+// Exact integer sums of the overscan columns of every frame, as per-block partials: block (c, k) writes the sum
+// of rows [256c, 256c + 256) of frame k to os_part[k * nos + c].  No atomics, so nothing has to be zeroed first;
+// the consumers add the nos = ceil(H/256) partials (integers: exact in any order).
+// Side job for the chained path: the blocks also clear `zero` (the accumulators of the kernels that follow on the
+// same stream), which saves the memset nodes between the stages.
+// grid (nos, n), block 256: one thread per row of the overscan strip
 // ---------------------------------------------------------------------------------------------
-// grid (ceil(H/256), n), block 256: one thread per row of the overscan strip
 __global__ void __launch_bounds__(256) k_frame_sums(const uint16_t* __restrict__ raw, Geom g, int n,
-                                                    unsigned long long* __restrict__ os_sum)
+                                                    unsigned long long* __restrict__ os_part,
+                                                    uint4* __restrict__ zero, size_t zero_n16)
 {
+    __shared__ unsigned long long s_w[8];
     const int k = blockIdx.y;
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (zero) {
+        const size_t tid = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
+        const size_t nth = (size_t)gridDim.x * gridDim.y * blockDim.x;
+        for (size_t i = tid; i < zero_n16; i += nth) zero[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
     unsigned long long s = 0;
-    if (r < g.H) s = overscan_row_sum(raw + (size_t)k * g.W * g.H, g.W, g.os_x0, g.os_x1, r);
+    if (r < g.H && g.os_x1 > g.os_x0) s = overscan_row_sum(raw + (size_t)k * g.W * g.H, g.W, g.os_x0, g.os_x1, r);
     s = warp_sum(s);
-    if ((threadIdx.x & 31) == 0 && s) atomicAdd(os_sum + k, s);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int i = 0; i < 8; ++i) t += s_w[i];
+        os_part[(size_t)k * gridDim.x + blockIdx.x] = t;
+    }
 }
 
-int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long long* os_sum,
-                      unsigned long long* /*img_sum*/, cudaStream_t st)
+int frame_sums_parts(const Geom& g) { return (g.H + 255) / 256; }
+
+int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long long* os_part, void* zero,
+                      size_t zero_bytes, cudaStream_t st)
 {
-    MRED_CUDA_TRY(cudaMemsetAsync(os_sum, 0, sizeof(unsigned long long) * n, st));
-    if (g.os_x1 <= g.os_x0) return MRED_OK;
-    dim3 grid((g.H + 255) / 256, n);
-    k_frame_sums<<<grid, 256, 0, st>>>(raw, g, n, os_sum);
+    dim3 grid(frame_sums_parts(g), n);
+    k_frame_sums<<<grid, 256, 0, st>>>(raw, g, n, os_part, static_cast<uint4*>(zero), zero ? zero_bytes / 16 : 0);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
+}
+
+// overscan level of frame k from the block partials (O1: exact integer sum, one float64 division)
+__device__ __forceinline__ double level_of(const unsigned long long* __restrict__ os_part, int nos, int k, const Geom& g)
+{
+    const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
+    unsigned long long t = 0;
+    for (int i = 0; i < nos; ++i) t += os_part[(size_t)k * nos + i];
+    return cnt > 0 ? (double)t / (double)cnt : 0.0;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -58,14 +82,13 @@ __device__ __forceinline__ void load4_u16(const uint16_t* p, int nv, float v[4])
 __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ raw, Geom g, int n, int fc,
                                                    float dark_scale, const float* __restrict__ MB,
                                                    const float* __restrict__ MD, const float* __restrict__ MF,
-                                                   float* __restrict__ out, const unsigned long long* __restrict__ os_sum,
-                                                   double* __restrict__ level_out, int vec_ok)
+                                                   float* __restrict__ out, const unsigned long long* __restrict__ os_part,
+                                                   int nos, double* __restrict__ level_out, int vec_ok)
 {
     __shared__ float s_level[CAL_MAXFC];
     const int k0 = blockIdx.y * fc, k1 = min(k0 + fc, n);
     if (threadIdx.x < k1 - k0) {
-        const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
-        const double L = cnt > 0 ? (double)os_sum[k0 + threadIdx.x] / (double)cnt : 0.0;
+        const double L = level_of(os_part, nos, k0 + threadIdx.x, g);
         s_level[threadIdx.x] = (float)L;
         if (level_out && blockIdx.x == 0) level_out[k0 + threadIdx.x] = L;
     }
@@ -130,18 +153,125 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// calibrate + marginal profiles in one pass (chained path, no bad-pixel mask): the calibrated pixels are summed
+// into the row / column profiles of O4 while they are still in registers, so estimate_shifts never re-reads the
+// calibrated stack (N*4wh bytes of HBM traffic and a kernel less; SURVEY 8(d) "0 if fused into calibrate").
+// Block = 512 threads = tile of 128 columns x 16 rows (warp = one 128-pixel row segment, lane = 4 pixels) of 4
+// frames; all loads of a thread are issued up front.  Row segment sums by warp shuffle; column sums over the 16
+// rows through shared memory (one barrier, then thread = (frame, column)); both are added to the global int64
+// fixed-point accumulators (value * 2^14) with integer atomics: exact and order-independent.
+// grid (ceil(w/128), ceil(h/16), ceil(n/4)).
+// ---------------------------------------------------------------------------------------------
+constexpr int CP_ROWS = 16, CP_COLS = 128, CP_FB = 4;     // tile and frames per block
+
+__global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __restrict__ raw, Geom g, int n,
+                                                           float dark_scale, const float* __restrict__ MB,
+                                                           const float* __restrict__ MD, const float* __restrict__ MF,
+                                                           float* __restrict__ out, const unsigned long long* __restrict__ os_part,
+                                                           int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
+                                                           int vec_ok)
+{
+    __shared__ float s_level[CP_FB];
+    __shared__ __align__(16) float s_col[CP_FB][CP_ROWS][CP_COLS];
+    const int k0 = blockIdx.z * CP_FB, nk = min(CP_FB, n - k0);
+    // (the last warp takes the levels: its float64 division then delays nobody else's loads)
+    if (threadIdx.x >= 512 - CP_FB && (int)threadIdx.x - (512 - CP_FB) < nk)
+        s_level[threadIdx.x - (512 - CP_FB)] = (float)level_of(os_part, nos, k0 + (int)threadIdx.x - (512 - CP_FB), g);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int x = blockIdx.x * CP_COLS + 4 * lane, y = blockIdx.y * CP_ROWS + warp;
+    const bool live = x < g.w && y < g.h;
+    const int nv = live ? min(4, g.w - x) : 0;
+    const bool vec = vec_ok && nv == 4;
+    const size_t p = live ? (size_t)y * g.w + x : 0;
+    const size_t fs = (size_t)g.W * g.H, np = (size_t)g.w * g.h;
+    // every global load of the thread is issued before the first barrier
+    float v[CP_FB][4];
+    {
+        const uint16_t* src = raw + (size_t)k0 * fs + (live ? (size_t)(y + g.y0) * g.W + g.x0 + x : 0);
+#pragma unroll
+        for (int j = 0; j < CP_FB; ++j) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) v[j][i] = 0.f;
+            if (j < nk && live) load4_u16(src + (size_t)j * fs, nv, v[j]);
+        }
+    }
+    float mb[4], ms[4], inv[4];
+    if (vec) {
+        const float4 a = __ldg(reinterpret_cast<const float4*>(MB + p));
+        const float4 b = __ldg(reinterpret_cast<const float4*>(MD + p));
+        const float4 c = __ldg(reinterpret_cast<const float4*>(MF + p));
+        mb[0] = a.x; mb[1] = a.y; mb[2] = a.z; mb[3] = a.w;
+        ms[0] = b.x; ms[1] = b.y; ms[2] = b.z; ms[3] = b.w;
+        inv[0] = c.x; inv[1] = c.y; inv[2] = c.z; inv[3] = c.w;
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            mb[i] = i < nv ? MB[p + i] : 0.f; ms[i] = i < nv ? MD[p + i] : 0.f; inv[i] = i < nv ? MF[p + i] : 0.f;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        mb[i] = fmaf(dark_scale, ms[i], mb[i]);
+        const float f = inv[i];
+        inv[i] = (f > 0.f && f <= 3.402823466e+38f) ? 1.0f / f : 0.f;     // dead lanes: 0, so they add nothing
+    }
+    float* dst = out + (size_t)k0 * np + p;
+#pragma unroll
+    for (int j = 0; j < CP_FB; ++j) {
+        if (j >= nk) break;                     // block-uniform
+        const float L = s_level[j];
+        float r[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) r[i] = ((v[j][i] - L) - mb[i]) * inv[i];
+        if (vec) __stcg(reinterpret_cast<float4*>(dst + (size_t)j * np), make_float4(r[0], r[1], r[2], r[3]));
+        else for (int i = 0; i < nv; ++i) dst[(size_t)j * np + i] = r[i];
+        *reinterpret_cast<float4*>(&s_col[j][warp][4 * lane]) = make_float4(r[0], r[1], r[2], r[3]);
+        const float rs = warp_sum((r[0] + r[1]) + (r[2] + r[3]));
+        if (lane == 0 && y < g.h)
+            atomicAdd(reinterpret_cast<unsigned long long*>(rowsum) + (size_t)(k0 + j) * g.h + y, (unsigned long long)__float2ll_rn(rs * PROF_FIX));
+    }
+    __syncthreads();
+    {   // 512 threads = 4 frames x 128 columns: 16 rows in a fixed order
+        const int j = threadIdx.x >> 7, c = threadIdx.x & (CP_COLS - 1);
+        const int cx = blockIdx.x * CP_COLS + c;
+        if (j < nk && cx < g.w) {
+            float t = 0.f;
+#pragma unroll
+            for (int rr = 0; rr < CP_ROWS; ++rr) t += s_col[j][rr][c];
+            atomicAdd(reinterpret_cast<unsigned long long*>(colsum) + (size_t)(k0 + j) * g.w + cx, (unsigned long long)__float2ll_rn(t * PROF_FIX));
+        }
+    }
+}
+
+// frames per chunk: enough chunks to fill the machine, at most 8 frames per thread, chunks of equal size
+static int chunk_frames(int n)
+{
+    const int nch = (n + 7) / 8;
+    return (n + nch - 1) / nch;
+}
+
+int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
+                          const float* MF, float* out, const unsigned long long* os_part, long long* colsum,
+                          long long* rowsum, cudaStream_t st)
+{
+    dim3 grid((unsigned)((g.w + CP_COLS - 1) / CP_COLS), (unsigned)((g.h + CP_ROWS - 1) / CP_ROWS), (unsigned)((n + CP_FB - 1) / CP_FB));
+    const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
+    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), colsum, rowsum, vec_ok);
+    MRED_LAUNCH_CHECK();
+    return MRED_OK;
+}
+
 int launch_calibrate(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
-                     const float* MF, float* out, double* level_out, const unsigned long long* os_sum,
-                     double* /*prof_ws*/, cudaStream_t st)
+                     const float* MF, float* out, double* level_out, const unsigned long long* os_part, cudaStream_t st)
 {
     const int w4 = (g.w + 3) / 4;
     const long long groups = (long long)g.h * w4;
-    // frames per chunk: enough chunks to fill the machine, at most CAL_MAXFC frames per thread
-    int fc = n < 8 ? n : 8;
-    if (fc > CAL_MAXFC) fc = CAL_MAXFC;
+    const int fc = chunk_frames(n);
     dim3 grid((unsigned)((groups + 255) / 256), (unsigned)((n + fc - 1) / fc));
     const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
-    k_calibrate<<<grid, 256, 0, st>>>(raw, g, n, fc, dark_scale, MB, MD, MF, out, os_sum, level_out, vec_ok);
+    k_calibrate<<<grid, 256, 0, st>>>(raw, g, n, fc, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), level_out, vec_ok);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }

@@ -42,6 +42,8 @@ void set_cuda_error(cudaError_t e);   // api.cu
 
 // Per-frame shifts / footprints handed over from the host by value (no allocation, no copy):
 // 255 frames x 16 B = 4080 B of kernel parameter space (sm_70+ allows 32 KB with CUDA >= 12.1).
+constexpr float PROF_FIX = 16384.0f;   // fixed-point scale of the profile sums of O4 (2^14: 6e-5 ADU per partial)
+
 struct HostShifts { double s[MRED_MAX_STACK][2]; };       // (sx, sy) as passed to mred_resample
 struct HostFootprints { int4 fp[MRED_MAX_STACK]; };       // {x_lo, x_hi, y_lo, y_hi}
 
@@ -98,20 +100,27 @@ __host__ __device__ inline void axis_footprint(int n, double s, int& lo, int& hi
 #endif
 
 // launchers implemented in the .cu files (all enqueue on `st`, return mred_status)
-int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long long* os_sum,
-                      unsigned long long* img_sum, cudaStream_t st);
+int frame_sums_parts(const Geom& g);      // partial sums per frame that launch_frame_sums writes (8 bytes each)
+int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long long* os_part, void* zero /* nullable */,
+                      size_t zero_bytes, cudaStream_t st);
 int launch_calibrate(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
-                     const float* MF, float* out, double* level_out, const unsigned long long* os_sum,
-                     double* prof_ws, cudaStream_t st);
+                     const float* MF, float* out, double* level_out, const unsigned long long* os_part, cudaStream_t st);
+int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
+                          const float* MF, float* out, const unsigned long long* os_part, long long* colsum,
+                          long long* rowsum, cudaStream_t st);
 int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint16_t* dark, int nd, float t_dark,
                          const uint16_t* flat, int nf, float t_flat, const mred_comb_opts& o, float* MB, float* MD,
                          float* MF, void* ws, cudaStream_t st);
 size_t masters_ws_bytes(const Geom& g, int n);
 int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host, const int32_t* fp_dev,
                  const mred_comb_opts& o, float* out, uint16_t* count, uint32_t* rejmask, cudaStream_t st);
+// stage flags of launch_estimate (chained path): accumulators already cleared / profile sums already accumulated
+enum { EST_ZEROED = 1, EST_HAVE_SUMS = 2 };
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
-                    int32_t* ishift, double* shift, void* ws, cudaStream_t st);
+                    int32_t* ishift, double* shift, void* ws, int flags, cudaStream_t st);
 size_t estimate_ws_bytes(int w, int h, int n);
+// the accumulators inside an estimate workspace: what has to be zero before the sums start, and where they are
+void estimate_accumulators(void* ws, int w, int h, int n, void** zero, size_t* zero_bytes, long long** colsum, long long** rowsum);
 int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,
                     const double* dshift_dev /* [n][2] (dx,dy): shift = -d */, float fill, float* out,
                     int32_t* fp_dev /* nullable */, void* ws /* nullable */, size_t ws_bytes, cudaStream_t st);

@@ -15,7 +15,7 @@ namespace mred {
 
 constexpr int PROF_BR = 32;        // rows per band
 constexpr int RIF = 4;             // rows in flight per thread in k_profiles
-constexpr float FIX = 16384.0f;    // fixed-point scale of the profile sums (2^14: 6e-5 ADU per partial)
+constexpr float FIX = PROF_FIX;    // fixed-point scale of the profile sums (common.cuh)
 constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
 
 struct EstimateWs {
@@ -26,7 +26,7 @@ struct EstimateWs {
     int* rowcnt;      // [n][h]
     double* prof;     // [n][2][plen]  median-subtracted profiles (x then y)
     double* corr;     // [n][2][2*MRED_MAX_LAG+1]  C(l) of every lag
-    size_t bytes;
+    size_t zero_bytes, bytes;
     int nbands, plen;
 };
 
@@ -42,6 +42,7 @@ static EstimateWs carve_est(void* ws, int w, int h, int n)
     e.ticket = reinterpret_cast<unsigned int*>(take(4 * (size_t)n * 2));
     e.rowsum = reinterpret_cast<long long*>(take(8 * (size_t)n * h));
     e.rowcnt = reinterpret_cast<int*>(take(4 * (size_t)n * h));
+    e.zero_bytes = (size_t)(p - static_cast<char*>(ws));    // everything up to here is an accumulator: cleared per call
     e.prof = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * e.plen));
     e.corr = reinterpret_cast<double*>(take(8 * (size_t)n * 2 * (2 * MRED_MAX_LAG + 1)));
     e.bytes = (size_t)(p - static_cast<char*>(ws));
@@ -49,6 +50,12 @@ static EstimateWs carve_est(void* ws, int w, int h, int n)
 }
 
 size_t estimate_ws_bytes(int w, int h, int n) { return carve_est(nullptr, w, h, n).bytes; }
+
+void estimate_accumulators(void* ws, int w, int h, int n, void** zero, size_t* zero_bytes, long long** colsum, long long** rowsum)
+{
+    const EstimateWs e = carve_est(ws, w, h, n);
+    *zero = e.colpart; *zero_bytes = e.zero_bytes; *colsum = e.colpart; *rowsum = e.rowsum;
+}
 
 __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ frames, int w, int h,
                                                   const uint8_t* __restrict__ bad, EstimateWs e, int vec_ok)
@@ -304,13 +311,15 @@ __global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref,
 }
 
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
-                    int32_t* ishift, double* shift, void* ws, cudaStream_t st)
+                    int32_t* ishift, double* shift, void* ws, int flags, cudaStream_t st)
 {
     const EstimateWs e = carve_est(ws, w, h, n);
     const int vec_ok = (w % 4 == 0) ? 1 : 0;
-    MRED_CUDA_TRY(cudaMemsetAsync(e.colpart, 0, (size_t)(reinterpret_cast<char*>(e.ticket) - reinterpret_cast<char*>(e.colpart)) + 4 * (size_t)n * 2, st));
-    k_profiles<<<dim3(e.nbands, n), 256, 0, st>>>(frames, w, h, bad, e, vec_ok);
-    MRED_LAUNCH_CHECK();
+    if (!(flags & EST_ZEROED)) MRED_CUDA_TRY(cudaMemsetAsync(e.colpart, 0, e.zero_bytes, st));
+    if (!(flags & EST_HAVE_SUMS)) {
+        k_profiles<<<dim3(e.nbands, n), 256, 0, st>>>(frames, w, h, bad, e, vec_ok);
+        MRED_LAUNCH_CHECK();
+    }
     int P = 1;
     while (P < (w > h ? w : h)) P <<= 1;
     static bool attr_done = false;   // idempotent

@@ -336,6 +336,31 @@ def _chain_check(grp, max_lag, mode, full_size=False):
     return e
 
 
+def test_reduce_fused_profiles_ragged_matches_unfused_route():
+    """Without a bad-pixel mask mred_reduce sums the marginal profiles inside the calibrate kernel (k_calibrate_prof,
+    128 x 16 tiles, 4 frames per block); with a mask it runs k_calibrate + k_profiles.  On a geometry with odd
+    W, odd x0, w % 4 != 0 and ragged tiles (183 x 71, 6 frames = 4 + 2) the two routes must give the same
+    integer shifts, the same sub-pixel shifts to 1e-6 px and the same co-add; an all-zero mask
+    changes nothing in the definition (O4), so the oracle chain is the reference for both."""
+    grp = synth.make_group(3, geom=GEOMS["ragged"], stars=25, S=5.0, n_sci=6, n_master=3)
+    g, n = grp.geom, grp.sci.shape[0]
+    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
+    c = oracle.calibrate(g, grp.sci, grp.t_sci / grp.t_dark, m.MB, m.MD, m.MF)
+    e = oracle.estimate_shifts(c.out, 0, 10)
+    MB, MD, MF = dev(m.MB.astype(np.float32)), dev(m.MD.astype(np.float32)), dev(m.MF.astype(np.float32))
+    res = []
+    for mask in (None, torch.zeros((g.h, g.w), dtype=torch.uint8, device="cuda")):
+        plan = mred.ReducePlan(g, n)
+        mred.reduce(plan, dev(grp.sci), grp.t_sci / grp.t_dark, MB, MD, MF, 0, 10, badmask=mask, mode=1)
+        res.append((host(plan.shift).copy(), host(plan.out).copy(), host(plan.count).copy()))
+    for sh, _, _ in res:
+        assert np.max(np.abs(sh - e.shift)) <= 1e-3, np.max(np.abs(sh - e.shift))
+        assert np.array_equal(np.floor(sh + 0.5).astype(np.int64), e.ishift.astype(np.int64))
+    assert np.max(np.abs(res[0][0] - res[1][0])) <= 1e-6
+    assert np.array_equal(res[0][2], res[1][2])
+    assert np.max(np.abs(res[0][1].astype(np.float64) - res[1][1])) <= 0.05     # shifts equal to 1e-6 px
+
+
 def test_reduce_chain_small():
     grp = synth.make_group(1, geom=synth.GEOM_SMALL, stars=30, S=6.0)
     _chain_check(grp, 12, 0)

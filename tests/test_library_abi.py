@@ -37,7 +37,7 @@ def test_host_only_calls(libpath):
     assert m.lib().mred_version().startswith(b"mred")
     assert m.lib().mred_strerror(-3) == b"workspace missing or too small"
     g = (1074, 1024, 0, 50, 50, 0, 1024, 1024)
-    assert m.workspace_bytes(m.CALL_CALIBRATE, g, 10) == 80
+    assert m.workspace_bytes(m.CALL_CALIBRATE, g, 10) == 10 * 4 * 8      # 4 block partials of the overscan sum per frame
     need = m.workspace_bytes(m.CALL_REDUCE, g, 10)
     assert need >= 2 * 10 * 1024 * 1024 * 4
     assert m.reduce_host_workspace_bytes(g, 10) >= need + 10 * 1074 * 1024 * 2
