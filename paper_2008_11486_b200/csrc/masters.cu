@@ -50,21 +50,23 @@ size_t masters_ws_bytes(const Geom& g, int n)
     return carve(nullptr, g, n, n, n).bytes;   // n = max(nb, nd, nf) is an upper bound for each
 }
 
-// Exact integer sums of all three stacks in one launch: overscan columns of every frame (blocks
-// x < nos: one thread per row), and the image rectangle of the flats for <F_k> (blocks x >= nos: one row per
-// warp, coalesced).  grid (nos + nimg, nb+nd+nf), block 256; integer atomics -> bit-exact.
+// Exact integer sums of all three stacks in one launch: overscan columns of every frame (the first nos * (nb+nd+nf)
+// blocks: one thread per row), and the image rectangle of the flats for <F_k> (the remaining nimg * nf blocks: one
+// row per warp, coalesced, 16 loads in flight per lane).  1-D grid, block 256; integer atomics -> bit-exact.
 __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict__ bias, int nb,
                                                      const uint16_t* __restrict__ dark, int nd,
-                                                     const uint16_t* __restrict__ flat, int nf, Geom g, int nos,
+                                                     const uint16_t* __restrict__ flat, int nf, Geom g, int nos, int nimg,
                                                      unsigned long long* __restrict__ os,
                                                      unsigned long long* __restrict__ img_f, int pair_ok)
 {
-    const int k = blockIdx.y;
     const size_t fs = (size_t)g.W * g.H;
-    const uint16_t* f = k < nb ? bias + (size_t)k * fs : (k < nb + nd ? dark + (size_t)(k - nb) * fs : flat + (size_t)(k - nb - nd) * fs);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if ((int)blockIdx.x < nos) {
-        const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nall = nb + nd + nf;
+    int b = blockIdx.x;
+    if (b < nos * nall) {
+        const int k = b / nos, c = b - k * nos;
+        const uint16_t* f = k < nb ? bias + (size_t)k * fs : (k < nb + nd ? dark + (size_t)(k - nb) * fs : flat + (size_t)(k - nb - nd) * fs);
+        const int r = c * blockDim.x + threadIdx.x;
         unsigned long long s = 0;
         if (r < g.H && g.os_x1 > g.os_x0) s = overscan_row_sum(f, g.W, g.os_x0, g.os_x1, r);
         s = warp_sum(s);
@@ -78,35 +80,39 @@ __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict_
         }
         return;
     }
-    if (k < nb + nd) return;                       // image sums: flats only
-    const int r = g.y0 + ((int)blockIdx.x - nos) * 8 + warp;
+    b -= nos * nall;                               // image sums: flats only
+    const int kf = b / nimg, c = b - kf * nimg;
+    const uint16_t* f = flat + (size_t)kf * fs;
+    const int r = g.y0 + c * 8 + warp;
     __shared__ unsigned long long s_b[8];
     const bool live = r < g.y0 + g.h;
     const uint16_t* row = f + (size_t)(live ? r : g.y0) * g.W;
-    unsigned long long b = 0;
+    unsigned long long bsum = 0;
     if (!live) {
-    } else if (pair_ok) {      // two pixels per 32-bit load, 8 independent loads in flight
+    } else if (pair_ok) {      // two pixels per 32-bit load, 16 independent loads in flight
         const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
         const int w2 = g.w >> 1;
         int x = lane;
-        for (; x + 7 * 32 < w2; x += 8 * 32) {
-            unsigned int v[8];
+        for (; x + 15 * 32 < w2; x += 16 * 32) {
+            unsigned int v[16];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) v[u] = __ldg(row2 + x + 32 * u);
+            for (int u = 0; u < 16; ++u) v[u] = __ldg(row2 + x + 32 * u);
+            unsigned int t = 0;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) b += (v[u] & 0xffffu) + (v[u] >> 16);
+            for (int u = 0; u < 16; ++u) t += (v[u] & 0xffffu) + (v[u] >> 16);     // 32 x 65535 < 2^32
+            bsum += t;
         }
-        for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); b += (v & 0xffffu) + (v >> 16); }
+        for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); bsum += (v & 0xffffu) + (v >> 16); }
     } else {
-        for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) b += __ldg(row + x);
+        for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) bsum += __ldg(row + x);
     }
-    b = warp_sum(b);
-    if (lane == 0) s_b[warp] = b;
+    bsum = warp_sum(bsum);
+    if (lane == 0) s_b[warp] = bsum;
     __syncthreads();
     if (threadIdx.x == 0) {
         unsigned long long t = 0;
         for (int i = 0; i < 8; ++i) t += s_b[i];
-        if (t) atomicAdd(img_f + (k - nb - nd), t);
+        if (t) atomicAdd(img_f + kf, t);
     }
 }
 
@@ -408,7 +414,7 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     // pairs of pixels by one 32-bit load need even W, x0 and w (frame bases are 16-byte aligned, frames W*H*2 B)
     const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0 && g.w % 2 == 0 && ((size_t)g.W * g.H) % 2 == 0) ? 1 : 0;
     const int nos = (g.H + 255) / 256, nimg = (g.h + 7) / 8;
-    k_master_sums<<<dim3(nos + nimg, nb + nd + nf), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, nos, m.os, m.img_f, pair_ok);
+    k_master_sums<<<dim3((unsigned)(nos * (nb + nd + nf) + nimg * nf)), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, nos, nimg, m.os, m.img_f, pair_ok);
     MRED_LAUNCH_CHECK();
     const size_t np = (size_t)g.w * g.h;
     const int nbd = nb > nd ? nb : nd;
@@ -416,7 +422,7 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     const double rd = (double)t_flat / (double)t_dark;
 #define CALL_BD(N, PX)                                                                                         \
     do {                                                                                                       \
-        if (PX == 2 && pair_ok && nb == N && nd == N) launch_bd<N, PX, true>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        if (PX == 2 && pair_ok && nb == N && nd == N) launch_bd<N, PX, PX == 2>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
         else if (PX == 2 && pair_ok) launch_bd<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
         else launch_bd<N, 1, false>(o.mode, dim3((unsigned)((np + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
     } while (0)
@@ -425,7 +431,7 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     MRED_LAUNCH_CHECK();
 #define CALL_F(N, PX)                                                                                          \
     do {                                                                                                       \
-        if (PX == 2 && pair_ok && nf == N) launch_f<N, PX, true>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        if (PX == 2 && pair_ok && nf == N) launch_f<N, PX, PX == 2>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
         else if (PX == 2 && pair_ok) launch_f<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
         else launch_f<N, 1, false>(o.mode, dim3((unsigned)((np + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
     } while (0)
