@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
 // frames; all loads of a thread are issued up front.  Row segment sums by warp shuffle; column sums over the 16
 // rows through shared memory (one barrier, then thread = (frame, column)); both are added to the global int64
 // fixed-point accumulators (value * 2^14) with integer atomics: exact and order-independent.
-// grid (ceil(n/4), ceil(w/128), ceil(h/(16 R))).
+// grid (ceil(n/4), ceil(w/128), ceil(h/16)).
 // ---------------------------------------------------------------------------------------------
 constexpr int CP_ROWS = 16, CP_COLS = 128, CP_FB = 4;     // tile and frames per block
 
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __res
                                                            const float* __restrict__ MD, const float* __restrict__ MF,
                                                            float* __restrict__ out, const unsigned long long* __restrict__ os_part,
                                                            int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
-                                                           int vec_ok, int R)
+                                                           int vec_ok)
 {
     __shared__ float s_level[CP_FB];
     __shared__ __align__(16) float s_col[CP_FB][CP_ROWS][CP_COLS];
@@ -181,78 +181,70 @@ __global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __res
     if (threadIdx.x >= 512 - CP_FB && (int)threadIdx.x - (512 - CP_FB) < nk)
         s_level[threadIdx.x - (512 - CP_FB)] = (float)level_of(os_part, nos, k0 + (int)threadIdx.x - (512 - CP_FB), g);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int x = blockIdx.y * CP_COLS + 4 * lane;
+    const int x = blockIdx.y * CP_COLS + 4 * lane, y = blockIdx.z * CP_ROWS + warp;
+    const bool live = x < g.w && y < g.h;
+    const int nv = live ? min(4, g.w - x) : 0;
+    const bool vec = vec_ok && nv == 4;
+    const size_t p = live ? (size_t)y * g.w + x : 0;
     const size_t fs = (size_t)g.W * g.H, np = (size_t)g.w * g.h;
-    const int cj = threadIdx.x >> 7, cc = threadIdx.x & (CP_COLS - 1);     // (frame, column) this thread reduces
-    const int cx = blockIdx.y * CP_COLS + cc;
-    long long colacc = 0;
-    // R tiles of 16 rows, one below the other: the column sums of a block cover 16 R rows, so a large stack issues
-    // R times fewer column atomics (R = 1 when the grid would otherwise not fill the machine)
-    for (int it = 0; it < R; ++it) {
-        const int ty = ((int)blockIdx.z * R + it) * CP_ROWS;
-        if (ty >= g.h) break;                       // block-uniform
-        const int y = ty + warp;
-        const bool live = x < g.w && y < g.h;
-        const int nv = live ? min(4, g.w - x) : 0;
-        const bool vec = vec_ok && nv == 4;
-        const size_t p = live ? (size_t)y * g.w + x : 0;
-        // every global load of the thread is issued before the barrier
-        float v[CP_FB][4];
-        {
-            const uint16_t* src = raw + (size_t)k0 * fs + (live ? (size_t)(y + g.y0) * g.W + g.x0 + x : 0);
-#pragma unroll
-            for (int j = 0; j < CP_FB; ++j) {
-#pragma unroll
-                for (int i = 0; i < 4; ++i) v[j][i] = 0.f;
-                if (j < nk && live) load4_u16(src + (size_t)j * fs, nv, v[j]);
-            }
-        }
-        float mb[4], ms[4], inv[4];
-        if (vec) {
-            const float4 a = __ldg(reinterpret_cast<const float4*>(MB + p));
-            const float4 b = __ldg(reinterpret_cast<const float4*>(MD + p));
-            const float4 c = __ldg(reinterpret_cast<const float4*>(MF + p));
-            mb[0] = a.x; mb[1] = a.y; mb[2] = a.z; mb[3] = a.w;
-            ms[0] = b.x; ms[1] = b.y; ms[2] = b.z; ms[3] = b.w;
-            inv[0] = c.x; inv[1] = c.y; inv[2] = c.z; inv[3] = c.w;
-        } else {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                mb[i] = i < nv ? MB[p + i] : 0.f; ms[i] = i < nv ? MD[p + i] : 0.f; inv[i] = i < nv ? MF[p + i] : 0.f;
-            }
-        }
-        __syncthreads();        // s_level written (first tile); everyone is done reading s_col of the previous tile
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            mb[i] = fmaf(dark_scale, ms[i], mb[i]);
-            const float f = inv[i];
-            inv[i] = (f > 0.f && f <= 3.402823466e+38f) ? 1.0f / f : 0.f;     // dead lanes: 0, so they add nothing
-        }
-        float* dst = out + (size_t)k0 * np + p;
+    // every global load of the thread is issued before the first barrier
+    float v[CP_FB][4];
+    {
+        const uint16_t* src = raw + (size_t)k0 * fs + (live ? (size_t)(y + g.y0) * g.W + g.x0 + x : 0);
 #pragma unroll
         for (int j = 0; j < CP_FB; ++j) {
-            if (j >= nk) break;                     // block-uniform
-            const float L = s_level[j];
-            float r[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) r[i] = ((v[j][i] - L) - mb[i]) * inv[i];
-            if (vec) __stcg(reinterpret_cast<float4*>(dst + (size_t)j * np), make_float4(r[0], r[1], r[2], r[3]));
-            else for (int i = 0; i < nv; ++i) dst[(size_t)j * np + i] = r[i];
-            *reinterpret_cast<float4*>(&s_col[j][warp][4 * lane]) = make_float4(r[0], r[1], r[2], r[3]);
-            const float rs = warp_sum((r[0] + r[1]) + (r[2] + r[3]));
-            if (lane == 0 && y < g.h)
-                atomicAdd(reinterpret_cast<unsigned long long*>(rowsum) + (size_t)(k0 + j) * g.h + y, (unsigned long long)__float2ll_rn(rs * PROF_FIX));
-        }
-        __syncthreads();
-        if (cj < nk && cx < g.w) {   // 512 threads = 4 frames x 128 columns: 16 rows in a fixed order
-            float t = 0.f;
-#pragma unroll
-            for (int rr = 0; rr < CP_ROWS; ++rr) t += s_col[cj][rr][cc];
-            colacc += __float2ll_rn(t * PROF_FIX);
+            for (int i = 0; i < 4; ++i) v[j][i] = 0.f;
+            if (j < nk && live) load4_u16(src + (size_t)j * fs, nv, v[j]);
         }
     }
-    if (cj < nk && cx < g.w)
-        atomicAdd(reinterpret_cast<unsigned long long*>(colsum) + (size_t)(k0 + cj) * g.w + cx, (unsigned long long)colacc);
+    float mb[4], ms[4], inv[4];
+    if (vec) {
+        const float4 a = __ldg(reinterpret_cast<const float4*>(MB + p));
+        const float4 b = __ldg(reinterpret_cast<const float4*>(MD + p));
+        const float4 c = __ldg(reinterpret_cast<const float4*>(MF + p));
+        mb[0] = a.x; mb[1] = a.y; mb[2] = a.z; mb[3] = a.w;
+        ms[0] = b.x; ms[1] = b.y; ms[2] = b.z; ms[3] = b.w;
+        inv[0] = c.x; inv[1] = c.y; inv[2] = c.z; inv[3] = c.w;
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            mb[i] = i < nv ? MB[p + i] : 0.f; ms[i] = i < nv ? MD[p + i] : 0.f; inv[i] = i < nv ? MF[p + i] : 0.f;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        mb[i] = fmaf(dark_scale, ms[i], mb[i]);
+        const float f = inv[i];
+        inv[i] = (f > 0.f && f <= 3.402823466e+38f) ? 1.0f / f : 0.f;     // dead lanes: 0, so they add nothing
+    }
+    float* dst = out + (size_t)k0 * np + p;
+#pragma unroll
+    for (int j = 0; j < CP_FB; ++j) {
+        if (j >= nk) break;                     // block-uniform
+        const float L = s_level[j];
+        float r[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) r[i] = ((v[j][i] - L) - mb[i]) * inv[i];
+        if (vec) __stcg(reinterpret_cast<float4*>(dst + (size_t)j * np), make_float4(r[0], r[1], r[2], r[3]));
+        else for (int i = 0; i < nv; ++i) dst[(size_t)j * np + i] = r[i];
+        *reinterpret_cast<float4*>(&s_col[j][warp][4 * lane]) = make_float4(r[0], r[1], r[2], r[3]);
+        const float rs = warp_sum((r[0] + r[1]) + (r[2] + r[3]));
+        if (lane == 0 && y < g.h)
+            atomicAdd(reinterpret_cast<unsigned long long*>(rowsum) + (size_t)(k0 + j) * g.h + y, (unsigned long long)__float2ll_rn(rs * PROF_FIX));
+    }
+    __syncthreads();
+    {   // 512 threads = 4 frames x 128 columns: 16 rows in a fixed order
+        const int j = threadIdx.x >> 7, c = threadIdx.x & (CP_COLS - 1);
+        const int cx = blockIdx.y * CP_COLS + c;
+        if (j < nk && cx < g.w) {
+            float t = 0.f;
+#pragma unroll
+            for (int rr = 0; rr < CP_ROWS; ++rr) t += s_col[j][rr][c];
+            atomicAdd(reinterpret_cast<unsigned long long*>(colsum) + (size_t)(k0 + j) * g.w + cx, (unsigned long long)__float2ll_rn(t * PROF_FIX));
+        }
+    }
 }
 
 // frames per chunk: enough chunks to fill the machine, at most 8 frames per thread, chunks of equal size
@@ -266,12 +258,11 @@ int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_
                           const float* MF, float* out, const unsigned long long* os_part, long long* colsum,
                           long long* rowsum, cudaStream_t st)
 {
-    const int tx = (g.w + CP_COLS - 1) / CP_COLS, ty = (g.h + CP_ROWS - 1) / CP_ROWS, ch = (n + CP_FB - 1) / CP_FB;
-    const int R = ((long long)tx * ty * ch >= 148LL * 3 * 8) ? 4 : 1;      // 4 tiles per block once that still leaves 2+ waves
-    if (tx > 65535 || (ty + R - 1) / R > 65535) return MRED_EINVAL;
-    dim3 grid((unsigned)ch, (unsigned)tx, (unsigned)((ty + R - 1) / R));
+    const int tx = (g.w + CP_COLS - 1) / CP_COLS, ty = (g.h + CP_ROWS - 1) / CP_ROWS;
+    if (tx > 65535 || ty > 65535) return MRED_EINVAL;
+    dim3 grid((unsigned)((n + CP_FB - 1) / CP_FB), (unsigned)tx, (unsigned)ty);
     const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
-    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), colsum, rowsum, vec_ok, R);
+    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), colsum, rowsum, vec_ok);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
