@@ -165,26 +165,27 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
 // ---------------------------------------------------------------------------------------------
 constexpr int CP_ROWS = 16, CP_COLS = 128, CP_FB = 4;     // tile and frames per block
 
-__global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __restrict__ raw, Geom g, int n,
-                                                           float dark_scale, const float* __restrict__ MB,
-                                                           const float* __restrict__ MD, const float* __restrict__ MF,
-                                                           float* __restrict__ out, const unsigned long long* __restrict__ os_part,
-                                                           int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
-                                                           int vec_ok)
+// FAST: the tile lies inside the image, holds 4 frames, rows are 16-byte aligned in the output and 4-byte aligned in
+// the raw frames: no per-thread bounds, tails or alignment tests (they were 40 % of the instructions issued).
+template <bool FAST>
+__device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__ raw, const Geom& g, int n,
+                                                    float dark_scale, const float* __restrict__ MB,
+                                                    const float* __restrict__ MD, const float* __restrict__ MF,
+                                                    float* __restrict__ out, const unsigned long long* __restrict__ os_part,
+                                                    int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
+                                                    int vec_ok, float (&s_level)[CP_FB], float (&s_col)[CP_FB][CP_ROWS][CP_COLS])
 {
-    __shared__ float s_level[CP_FB];
-    __shared__ __align__(16) float s_col[CP_FB][CP_ROWS][CP_COLS];
     // blockIdx.x = frame chunk (fastest): the blocks that share a tile of the master planes run together, so the
     // masters come out of HBM once and out of L2 for the other chunks (they exceed L2 at 4096^2)
-    const int k0 = blockIdx.x * CP_FB, nk = min(CP_FB, n - k0);
+    const int k0 = blockIdx.x * CP_FB, nk = FAST ? CP_FB : min(CP_FB, n - k0);
     // (the last warp takes the levels: its float64 division then delays nobody else's loads)
     if (threadIdx.x >= 512 - CP_FB && (int)threadIdx.x - (512 - CP_FB) < nk)
         s_level[threadIdx.x - (512 - CP_FB)] = (float)level_of(os_part, nos, k0 + (int)threadIdx.x - (512 - CP_FB), g);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x = blockIdx.y * CP_COLS + 4 * lane, y = blockIdx.z * CP_ROWS + warp;
-    const bool live = x < g.w && y < g.h;
-    const int nv = live ? min(4, g.w - x) : 0;
-    const bool vec = vec_ok && nv == 4;
+    const bool live = FAST || (x < g.w && y < g.h);
+    const int nv = FAST ? 4 : (live ? min(4, g.w - x) : 0);
+    const bool vec = FAST || (vec_ok && nv == 4);
     const size_t p = live ? (size_t)y * g.w + x : 0;
     const size_t fs = (size_t)g.W * g.H, np = (size_t)g.w * g.h;
     // every global load of the thread is issued before the first barrier
@@ -195,7 +196,14 @@ __global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __res
         for (int j = 0; j < CP_FB; ++j) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) v[j][i] = 0.f;
-            if (j < nk && live) load4_u16(src + (size_t)j * fs, nv, v[j]);
+            if (FAST) {
+                const unsigned int* q = reinterpret_cast<const unsigned int*>(src + (size_t)j * fs);
+                const unsigned int a = __ldcs(q), b = __ldcs(q + 1);
+                v[j][0] = (float)(a & 0xffffu); v[j][1] = (float)(a >> 16);
+                v[j][2] = (float)(b & 0xffffu); v[j][3] = (float)(b >> 16);
+            } else if (j < nk && live) {
+                load4_u16(src + (size_t)j * fs, nv, v[j]);
+            }
         }
     }
     float mb[4], ms[4], inv[4];
@@ -231,20 +239,35 @@ __global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __res
         else for (int i = 0; i < nv; ++i) dst[(size_t)j * np + i] = r[i];
         *reinterpret_cast<float4*>(&s_col[j][warp][4 * lane]) = make_float4(r[0], r[1], r[2], r[3]);
         const float rs = warp_sum((r[0] + r[1]) + (r[2] + r[3]));
-        if (lane == 0 && y < g.h)
+        if (lane == 0 && (FAST || y < g.h))
             atomicAdd(reinterpret_cast<unsigned long long*>(rowsum) + (size_t)(k0 + j) * g.h + y, (unsigned long long)__float2ll_rn(rs * PROF_FIX));
     }
     __syncthreads();
     {   // 512 threads = 4 frames x 128 columns: 16 rows in a fixed order
         const int j = threadIdx.x >> 7, c = threadIdx.x & (CP_COLS - 1);
         const int cx = blockIdx.y * CP_COLS + c;
-        if (j < nk && cx < g.w) {
+        if (FAST || (j < nk && cx < g.w)) {
             float t = 0.f;
 #pragma unroll
             for (int rr = 0; rr < CP_ROWS; ++rr) t += s_col[j][rr][c];
             atomicAdd(reinterpret_cast<unsigned long long*>(colsum) + (size_t)(k0 + j) * g.w + cx, (unsigned long long)__float2ll_rn(t * PROF_FIX));
         }
     }
+}
+
+__global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __restrict__ raw, Geom g, int n,
+                                                           float dark_scale, const float* __restrict__ MB,
+                                                           const float* __restrict__ MD, const float* __restrict__ MF,
+                                                           float* __restrict__ out, const unsigned long long* __restrict__ os_part,
+                                                           int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
+                                                           int vec_ok, int pair_ok)
+{
+    __shared__ float s_level[CP_FB];
+    __shared__ __align__(16) float s_col[CP_FB][CP_ROWS][CP_COLS];
+    const bool fast = vec_ok && pair_ok && (int)(blockIdx.x + 1) * CP_FB <= n && (int)(blockIdx.y + 1) * CP_COLS <= g.w &&
+                      (int)(blockIdx.z + 1) * CP_ROWS <= g.h;      // block-uniform
+    if (fast) calibrate_prof_body<true>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, colsum, rowsum, vec_ok, s_level, s_col);
+    else calibrate_prof_body<false>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, colsum, rowsum, vec_ok, s_level, s_col);
 }
 
 // frames per chunk: enough chunks to fill the machine, at most 8 frames per thread, chunks of equal size
@@ -262,7 +285,8 @@ int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_
     if (tx > 65535 || ty > 65535) return MRED_EINVAL;
     dim3 grid((unsigned)((n + CP_FB - 1) / CP_FB), (unsigned)tx, (unsigned)ty);
     const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
-    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), colsum, rowsum, vec_ok);
+    const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0) ? 1 : 0;     // raw rows of the image rectangle start 4-byte aligned
+    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), colsum, rowsum, vec_ok, pair_ok);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
