@@ -23,12 +23,12 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
     // Classify every frame against the block's 256 consecutive pixels: footprint covers all of them (the
     // usual case: bit in s_in, no per-pixel test), none of them, or some (bit in s_part: per-pixel test).
     {
-        const size_t p0 = (size_t)blockIdx.x * blockDim.x;
-        const size_t p1 = min(p0 + blockDim.x, np) - 1;
-        const int ya = (int)((unsigned)p0 / (unsigned)w), yb = (int)((unsigned)p1 / (unsigned)w);   // w*h < 2^31 (api.cu)
-        const int xa = (int)(p0 - (size_t)ya * w), xb = (int)(p1 - (size_t)yb * w);
         const int k = threadIdx.x;
-        if (k < NW * 32) {
+        if (k < NW * 32) {          // only these warps pay for the two integer divisions
+            const size_t p0 = (size_t)blockIdx.x * blockDim.x;
+            const size_t p1 = min(p0 + blockDim.x, np) - 1;
+            const int ya = (int)((unsigned)p0 / (unsigned)w), yb = (int)((unsigned)p1 / (unsigned)w);   // w*h < 2^31 (api.cu)
+            const int xa = (int)(p0 - (size_t)ya * w), xb = (int)(p1 - (size_t)yb * w);
             int cls = 0;                                   // 0 none, 1 all, 2 some
             if (k < n) {
                 int4 f = make_int4(0, w - 1, 0, h - 1);
@@ -49,7 +49,6 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
     }
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
-    const int y = (int)((unsigned)p / (unsigned)w), x = (int)((unsigned)p - (unsigned)y * (unsigned)w);
     const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
     float v[NMAX];
     uint32_t inside[NW];
@@ -58,7 +57,8 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
 #pragma unroll
     for (int i = 0; i < NW; ++i) {
         uint32_t part = s_part[i];
-        while (part) {                                     // block-uniform, rarely non-zero
+        while (part) {                                     // block-uniform, rarely non-zero (footprint edges): the pixel's
+            const int y = (int)((unsigned)p / (unsigned)w), x = (int)((unsigned)p - (unsigned)y * (unsigned)w);   // (x, y) only here
             const int b = __ffs(part) - 1;
             part &= part - 1;
             const int4 f = s_fp[32 * i + b];
