@@ -91,7 +91,8 @@ int mred_build_masters(const mred_geom *geom, const uint16_t *bias, int nb, cons
  *     out_k = (raw_k - L_k - MB - dark_scale * MD) / MF   on the image rectangle;  MF <= 0 or
  *     non-finite -> 0.   dark_scale = t_sci / t_dark.
  * raw: uint16 [n][H][W]; out: float32 [n][h][w]; level_out: float64 [n] (device, nullable)
- * receives L_k.  n >= 1 (no upper bound other than memory).
+ * receives L_k.  n >= 1 (no upper bound other than memory).  ws holds ceil(H/256) partial overscan
+ * sums per frame (mred_workspace_bytes).
  */
 int mred_calibrate(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
                    const float *MD, const float *MF, float *out, double *level_out, void *ws, size_t ws_bytes,
@@ -141,6 +142,8 @@ int mred_coadd(const float *stack, int n, int w, int h, const int32_t *footprint
 /*
  * The whole science path for one group, device-resident and chained without host round trips:
  * calibrate -> estimate_shifts (vs ref_index) -> resample by (-dx, -dy) -> coadd.
+ * Without a badmask the marginal profiles of estimate_shifts are summed inside the calibrate kernel
+ * (same definition, O4; the calibrated stack is not read a second time).
  * raw: uint16 [n][H][W].  shift_out: float64 [n][2] device (nullable) receives (dx, dy);
  * footprint_out: int32 [n][4] device (nullable).  Other arguments as in the single calls.
  */
