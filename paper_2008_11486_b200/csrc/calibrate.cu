@@ -165,9 +165,10 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
 // ---------------------------------------------------------------------------------------------
 constexpr int CP_ROWS = 16, CP_COLS = 128, CP_FB = 4;     // tile and frames per block
 
-// FAST: the tile lies inside the image, holds 4 frames, rows are 16-byte aligned in the output and 4-byte aligned in
-// the raw frames: no per-thread bounds, tails or alignment tests (they were 40 % of the instructions issued).
-template <bool FAST>
+// NKF > 0 (fast body): the tile lies inside the image, holds exactly NKF frames, rows are 16-byte aligned in the
+// output and 4-byte aligned in the raw frames: no per-thread bounds, tails or alignment tests (they were 40 % of the
+// instructions issued).  NKF = 0: the general body.
+template <int NKF>
 __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__ raw, const Geom& g, int n,
                                                     float dark_scale, const float* __restrict__ MB,
                                                     const float* __restrict__ MD, const float* __restrict__ MF,
@@ -175,9 +176,10 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
                                                     int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
                                                     int vec_ok, float (&s_level)[CP_FB], float (&s_col)[CP_FB][CP_ROWS][CP_COLS])
 {
+    constexpr bool FAST = NKF > 0;
     // blockIdx.x = frame chunk (fastest): the blocks that share a tile of the master planes run together, so the
     // masters come out of HBM once and out of L2 for the other chunks (they exceed L2 at 4096^2)
-    const int k0 = blockIdx.x * CP_FB, nk = FAST ? CP_FB : min(CP_FB, n - k0);
+    const int k0 = blockIdx.x * CP_FB, nk = FAST ? NKF : min(CP_FB, n - k0);
     // (the last warp takes the levels: its float64 division then delays nobody else's loads)
     if (threadIdx.x >= 512 - CP_FB && (int)threadIdx.x - (512 - CP_FB) < nk)
         s_level[threadIdx.x - (512 - CP_FB)] = (float)level_of(os_part, nos, k0 + (int)threadIdx.x - (512 - CP_FB), g);
@@ -196,12 +198,12 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
         for (int j = 0; j < CP_FB; ++j) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) v[j][i] = 0.f;
-            if (FAST) {
+            if (FAST && j < NKF) {
                 const unsigned int* q = reinterpret_cast<const unsigned int*>(src + (size_t)j * fs);
                 const unsigned int a = __ldcs(q), b = __ldcs(q + 1);
                 v[j][0] = (float)(a & 0xffffu); v[j][1] = (float)(a >> 16);
                 v[j][2] = (float)(b & 0xffffu); v[j][3] = (float)(b >> 16);
-            } else if (j < nk && live) {
+            } else if (!FAST && j < nk && live) {
                 load4_u16(src + (size_t)j * fs, nv, v[j]);
             }
         }
@@ -246,7 +248,7 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
     {   // 512 threads = 4 frames x 128 columns: 16 rows in a fixed order
         const int j = threadIdx.x >> 7, c = threadIdx.x & (CP_COLS - 1);
         const int cx = blockIdx.y * CP_COLS + c;
-        if (FAST || (j < nk && cx < g.w)) {
+        if (FAST ? (j < NKF) : (j < nk && cx < g.w)) {
             float t = 0.f;
 #pragma unroll
             for (int rr = 0; rr < CP_ROWS; ++rr) t += s_col[j][rr][c];
@@ -264,10 +266,17 @@ __global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __res
 {
     __shared__ float s_level[CP_FB];
     __shared__ __align__(16) float s_col[CP_FB][CP_ROWS][CP_COLS];
-    const bool fast = vec_ok && pair_ok && (int)(blockIdx.x + 1) * CP_FB <= n && (int)(blockIdx.y + 1) * CP_COLS <= g.w &&
-                      (int)(blockIdx.z + 1) * CP_ROWS <= g.h;      // block-uniform
-    if (fast) calibrate_prof_body<true>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, colsum, rowsum, vec_ok, s_level, s_col);
-    else calibrate_prof_body<false>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, colsum, rowsum, vec_ok, s_level, s_col);
+    const bool fast = vec_ok && pair_ok && (int)(blockIdx.y + 1) * CP_COLS <= g.w && (int)(blockIdx.z + 1) * CP_ROWS <= g.h;
+    const int nkf = fast ? min(CP_FB, n - (int)blockIdx.x * CP_FB) : 0;      // block-uniform
+#define MRED_CP_BODY(N) calibrate_prof_body<N>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, colsum, rowsum, vec_ok, s_level, s_col)
+    switch (nkf) {
+        case 4: MRED_CP_BODY(4); break;
+        case 3: MRED_CP_BODY(3); break;
+        case 2: MRED_CP_BODY(2); break;
+        case 1: MRED_CP_BODY(1); break;
+        default: MRED_CP_BODY(0); break;
+    }
+#undef MRED_CP_BODY
 }
 
 // frames per chunk: enough chunks to fill the machine, at most 8 frames per thread, chunks of equal size
