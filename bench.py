@@ -208,7 +208,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 KERNELS_PER_BUILD_MASTERS = 4    # k_master_sums, k_masters_bd, k_masters_f, k_mf_scale
 KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd (+1: small stacks resample in two kernels); memset nodes not counted
-KERNELS_PER_REDUCE_FUSED = 6     # without a bad-pixel mask k_calibrate_prof replaces k_calibrate + k_profiles
+KERNELS_PER_REDUCE_FUSED = 6     # mred_reduce: k_calibrate_prof replaces k_calibrate + k_profiles (+1 with a bad-pixel mask: k_mask_counts)
 
 
 def run_ours(args):
@@ -340,7 +340,8 @@ def run_ours(args):
     value = frames_per_step * args.steps / (total_ms * 1e-3)
 
     # per-stage device times inside the timed region (average per call = per group)
-    fused = all(b is None for b in bad)
+    fused = True                     # mred_reduce always sums the profiles inside the calibrate kernel
+    masked = any(b is not None for b in bad)
     sb = stage_bytes(g, n, nm, words, fused_profiles=fused)
     st_ms = {k: [] for k in ["build_masters"] + STAGES}
     for evm, evs in stage_ev:
@@ -389,7 +390,7 @@ def run_ours(args):
     ref_stages = stages_iso if stages_iso is not None else stages
     dom = max(STAGES, key=lambda k: ref_stages[k]["ms_per_call"])
     kern = {"calibrate": ("k_calibrate_prof" if fused else "k_calibrate") + " (+k_frame_sums)",
-            "estimate_shifts": "k_finalize, k_correlate (profile sums come from k_calibrate_prof)" if fused else "k_profiles (+k_finalize, k_correlate)",
+            "estimate_shifts": "k_finalize, k_correlate (profile sums come from k_calibrate_prof)",
             "resample": "k_resample<1> + k_ypass4 (x pass, y pass)" if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else "k_resample<0>",
             "coadd": "k_coadd"}[dom]
     traffic = None
@@ -483,7 +484,7 @@ def run_ours(args):
                            "coadd": ["median", "mean", "sigclip 3.0 x3"][mode], "l2": "512 MB flush before every step",
                            "parallelism": "groups sharded over ranks, no collective", "streams": len(streams), "launch": "cuda graph replay" if graph is not None else "plain launches",
                            "stage_timing": "CUDA events inside the C call; with a graph: instrumented plain-launch passes of the same step right after the timed region"},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + (KERNELS_PER_REDUCE_FUSED if fused else KERNELS_PER_REDUCE) + (1 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 0)),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + (KERNELS_PER_REDUCE_FUSED + (1 if masked else 0)) + (1 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 0)),
                 "roofline": roof, "stages": stages, "stages_isolated": stages_iso, "path_roofline": e2e_roof, "cpu_baseline": cpu,
                 "wall_s_timed_region": round(wall, 4), "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU "
                 "stages on a TITAN X (Pascal) = ~870 frames/s (other hardware, other data; context only)"}

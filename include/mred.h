@@ -142,8 +142,8 @@ int mred_coadd(const float *stack, int n, int w, int h, const int32_t *footprint
 /*
  * The whole science path for one group, device-resident and chained without host round trips:
  * calibrate -> estimate_shifts (vs ref_index) -> resample by (-dx, -dy) -> coadd.
- * Without a badmask the marginal profiles of estimate_shifts are summed inside the calibrate kernel
- * (same definition, O4; the calibrated stack is not read a second time).
+ * The marginal profiles of estimate_shifts are summed inside the calibrate kernel (same definition,
+ * DESIGN.md O4, masked pixels left out; the calibrated stack is not read a second time).
  * raw: uint16 [n][H][W].  shift_out: float64 [n][2] device (nullable) receives (dx, dy);
  * footprint_out: int32 [n][4] device (nullable).  Other arguments as in the single calls.
  */

@@ -214,21 +214,20 @@ int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float 
 #define MRED_STAGE_EVENT(i) \
     do { if (events && events[i]) MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[i]), st)); } while (0)
     MRED_STAGE_EVENT(0);
-    // The level kernel also clears the accumulators of estimate_shifts (no memset node between the stages); without
-    // a bad-pixel mask the calibrate kernel sums the marginal profiles itself, so estimate_shifts starts at its
-    // finalize kernel and the calibrated stack is not re-read.
+    // The level kernel also clears the accumulators of estimate_shifts (no memset node between the stages); the
+    // calibrate kernel sums the marginal profiles itself (leaving out masked pixels), so estimate_shifts starts at
+    // its finalize kernel and the calibrated stack is not re-read.
     void* zero;
     size_t zero_bytes;
     long long *colsum, *rowsum;
     estimate_accumulators(r.est, g.w, g.h, n, &zero, &zero_bytes, &colsum, &rowsum);
     if ((rc = launch_frame_sums(raw, g, n, r.os, zero, zero_bytes, st))) return rc;
-    int est_flags = EST_ZEROED;
-    if (!badmask) {
-        if ((rc = launch_calibrate_prof(raw, g, n, dark_scale, MB, MD, MF, r.cal, r.os, colsum, rowsum, st))) return rc;
-        est_flags |= EST_HAVE_SUMS;
-    } else {
-        if ((rc = launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, r.cal, nullptr, r.os, st))) return rc;
+    int est_flags = EST_ZEROED | EST_HAVE_SUMS;
+    if (badmask) {      // the mask is the same for every frame: its valid-pixel counts are taken once
+        if ((rc = launch_mask_counts(badmask, g.w, g.h, n, r.est, st))) return rc;
+        est_flags |= EST_SHARED_COUNTS;
     }
+    if ((rc = launch_calibrate_prof(raw, g, n, dark_scale, MB, MD, MF, r.cal, r.os, badmask, colsum, rowsum, st))) return rc;
     MRED_STAGE_EVENT(1);
     double* shift = shift_out ? shift_out : r.shift;
     int32_t* fp = footprint_out ? footprint_out : r.fp;

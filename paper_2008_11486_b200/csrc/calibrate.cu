@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------------------------
-// calibrate + marginal profiles in one pass (chained path, no bad-pixel mask): the calibrated pixels are summed
+// calibrate + marginal profiles in one pass (chained path; an optional bad-pixel mask keeps pixels out of the sums): the calibrated pixels are summed
 // into the row / column profiles of O4 while they are still in registers, so estimate_shifts never re-reads the
 // calibrated stack (N*4wh bytes of HBM traffic and a kernel less; SURVEY 8(d) "0 if fused into calibrate").
 // Block = 512 threads = tile of 128 columns x 16 rows (warp = one 128-pixel row segment, lane = 4 pixels) of 4
@@ -168,13 +168,14 @@ constexpr int CP_ROWS = 16, CP_COLS = 128, CP_FB = 4;     // tile and frames per
 // NKF > 0 (fast body): the tile lies inside the image, holds exactly NKF frames, rows are 16-byte aligned in the
 // output and 4-byte aligned in the raw frames: no per-thread bounds, tails or alignment tests (they were 40 % of the
 // instructions issued).  NKF = 0: the general body.
-template <int NKF>
+template <int NKF, bool MASK>
 __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__ raw, const Geom& g, int n,
                                                     float dark_scale, const float* __restrict__ MB,
                                                     const float* __restrict__ MD, const float* __restrict__ MF,
                                                     float* __restrict__ out, const unsigned long long* __restrict__ os_part,
-                                                    int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
-                                                    int vec_ok, float (&s_level)[CP_FB], float (&s_col)[CP_FB][CP_ROWS][CP_COLS])
+                                                    int nos, const uint8_t* __restrict__ bad, long long* __restrict__ colsum,
+                                                    long long* __restrict__ rowsum, int vec_ok, float (&s_level)[CP_FB],
+                                                    float (&s_col)[CP_FB][CP_ROWS][CP_COLS])
 {
     constexpr bool FAST = NKF > 0;
     // blockIdx.x = frame chunk (fastest): the blocks that share a tile of the master planes run together, so the
@@ -222,6 +223,16 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
             mb[i] = i < nv ? MB[p + i] : 0.f; ms[i] = i < nv ? MD[p + i] : 0.f; inv[i] = i < nv ? MF[p + i] : 0.f;
         }
     }
+    unsigned okm = 0xfu;          // bit i: pixel i counts in the profiles (bad-pixel mask, O4)
+    if (MASK) {
+        if (vec) {
+            const uchar4 b = __ldg(reinterpret_cast<const uchar4*>(bad + p));
+            okm = (b.x ? 0u : 1u) | (b.y ? 0u : 2u) | (b.z ? 0u : 4u) | (b.w ? 0u : 8u);
+        } else {
+            okm = 0u;
+            for (int i = 0; i < nv; ++i) okm |= __ldg(bad + p + i) ? 0u : (1u << i);
+        }
+    }
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -239,6 +250,10 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
         for (int i = 0; i < 4; ++i) r[i] = ((v[j][i] - L) - mb[i]) * inv[i];
         if (vec) __stcg(reinterpret_cast<float4*>(dst + (size_t)j * np), make_float4(r[0], r[1], r[2], r[3]));
         else for (int i = 0; i < nv; ++i) dst[(size_t)j * np + i] = r[i];
+        if (MASK && okm != 0xfu) {  // masked pixels are written like any other but stay out of the profiles
+#pragma unroll
+            for (int i = 0; i < 4; ++i) r[i] = ((okm >> i) & 1u) ? r[i] : 0.f;
+        }
         *reinterpret_cast<float4*>(&s_col[j][warp][4 * lane]) = make_float4(r[0], r[1], r[2], r[3]);
         const float rs = warp_sum((r[0] + r[1]) + (r[2] + r[3]));
         if (lane == 0 && (FAST || y < g.h))
@@ -261,14 +276,18 @@ __global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __res
                                                            float dark_scale, const float* __restrict__ MB,
                                                            const float* __restrict__ MD, const float* __restrict__ MF,
                                                            float* __restrict__ out, const unsigned long long* __restrict__ os_part,
-                                                           int nos, long long* __restrict__ colsum, long long* __restrict__ rowsum,
-                                                           int vec_ok, int pair_ok)
+                                                           int nos, const uint8_t* __restrict__ bad, long long* __restrict__ colsum,
+                                                           long long* __restrict__ rowsum, int vec_ok, int pair_ok)
 {
     __shared__ float s_level[CP_FB];
     __shared__ __align__(16) float s_col[CP_FB][CP_ROWS][CP_COLS];
     const bool fast = vec_ok && pair_ok && (int)(blockIdx.y + 1) * CP_COLS <= g.w && (int)(blockIdx.z + 1) * CP_ROWS <= g.h;
     const int nkf = fast ? min(CP_FB, n - (int)blockIdx.x * CP_FB) : 0;      // block-uniform
-#define MRED_CP_BODY(N) calibrate_prof_body<N>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, colsum, rowsum, vec_ok, s_level, s_col)
+#define MRED_CP_BODY(N)                                                                                                                   \
+    do {                                                                                                                                  \
+        if (bad) calibrate_prof_body<N, true>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, bad, colsum, rowsum, vec_ok, s_level, s_col);  \
+        else calibrate_prof_body<N, false>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, nos, bad, colsum, rowsum, vec_ok, s_level, s_col);   \
+    } while (0)
     switch (nkf) {
         case 4: MRED_CP_BODY(4); break;
         case 3: MRED_CP_BODY(3); break;
@@ -287,15 +306,15 @@ static int chunk_frames(int n)
 }
 
 int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
-                          const float* MF, float* out, const unsigned long long* os_part, long long* colsum,
-                          long long* rowsum, cudaStream_t st)
+                          const float* MF, float* out, const unsigned long long* os_part, const uint8_t* bad,
+                          long long* colsum, long long* rowsum, cudaStream_t st)
 {
     const int tx = (g.w + CP_COLS - 1) / CP_COLS, ty = (g.h + CP_ROWS - 1) / CP_ROWS;
     if (tx > 65535 || ty > 65535) return MRED_EINVAL;
     dim3 grid((unsigned)((n + CP_FB - 1) / CP_FB), (unsigned)tx, (unsigned)ty);
     const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
     const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0) ? 1 : 0;     // raw rows of the image rectangle start 4-byte aligned
-    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), colsum, rowsum, vec_ok, pair_ok);
+    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), bad, colsum, rowsum, vec_ok, pair_ok);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }

@@ -106,8 +106,8 @@ int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long l
 int launch_calibrate(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
                      const float* MF, float* out, double* level_out, const unsigned long long* os_part, cudaStream_t st);
 int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_scale, const float* MB, const float* MD,
-                          const float* MF, float* out, const unsigned long long* os_part, long long* colsum,
-                          long long* rowsum, cudaStream_t st);
+                          const float* MF, float* out, const unsigned long long* os_part, const uint8_t* bad /* nullable */,
+                          long long* colsum, long long* rowsum, cudaStream_t st);
 int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint16_t* dark, int nd, float t_dark,
                          const uint16_t* flat, int nf, float t_flat, const mred_comb_opts& o, float* MB, float* MD,
                          float* MF, void* ws, cudaStream_t st);
@@ -115,7 +115,8 @@ size_t masters_ws_bytes(const Geom& g, int n);
 int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host, const int32_t* fp_dev,
                  const mred_comb_opts& o, float* out, uint16_t* count, uint32_t* rejmask, cudaStream_t st);
 // stage flags of launch_estimate (chained path): accumulators already cleared / profile sums already accumulated
-enum { EST_ZEROED = 1, EST_HAVE_SUMS = 2 };
+enum { EST_ZEROED = 1, EST_HAVE_SUMS = 2, EST_SHARED_COUNTS = 4 };   // 4: valid-pixel counts of the mask in frame 0's arrays (launch_mask_counts)
+int launch_mask_counts(const uint8_t* bad, int w, int h, int n, void* ws, cudaStream_t st);
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
                     int32_t* ishift, double* shift, void* ws, int flags, cudaStream_t st);
 size_t estimate_ws_bytes(int w, int h, int n);

@@ -135,6 +135,28 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
     }
 }
 
+// Valid-pixel counts per column and per row of the bad-pixel mask, into the count arrays of frame 0 (the mask is the
+// same for every frame of a stack, so the chained path counts once and k_finalize reads frame 0's counts for all frames).
+// grid (nbands), block 256; the arrays must be zero on entry.
+__global__ void __launch_bounds__(256) k_mask_counts(const uint8_t* __restrict__ bad, int w, int h, EstimateWs e)
+{
+    const int y0 = blockIdx.x * PROF_BR, y1 = min(y0 + PROF_BR, h);
+    const int lane = threadIdx.x & 31;
+    for (int xc = 0; xc < w; xc += 1024) {
+        const int x = xc + 4 * threadIdx.x;
+        const int nv = max(0, min(4, w - x));
+        int cc[4] = {0, 0, 0, 0};
+        for (int y = y0; y < y1; ++y) {
+            int rc = 0;
+            for (int i = 0; i < nv; ++i) { const int ok = !__ldg(bad + (size_t)y * w + x + i); cc[i] += ok; rc += ok; }
+            rc = warp_sum(rc);
+            if (lane == 0 && rc) atomicAdd(e.rowcnt + y, rc);
+        }
+        for (int i = 0; i < nv; ++i)
+            if (cc[i]) atomicAdd(e.colcnt + x + i, cc[i]);
+    }
+}
+
 // order-preserving map double -> uint64
 __device__ __forceinline__ unsigned long long key_of(double v)
 {
@@ -205,10 +227,10 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
             int c = axis == 0 ? h : w;         // without a bad-pixel mask every line is complete
             if (axis == 0) {
                 s = __ldcg(e.colpart + (size_t)k * w + i);
-                if (has_bad) c = __ldcg(e.colcnt + (size_t)k * w + i);
+                if (has_bad) c = __ldcg(e.colcnt + (size_t)(has_bad == 2 ? 0 : k) * w + i);
             } else {
                 s = __ldcg(e.rowsum + (size_t)k * h + i);
-                if (has_bad) c = __ldcg(e.rowcnt + (size_t)k * h + i);
+                if (has_bad) c = __ldcg(e.rowcnt + (size_t)(has_bad == 2 ? 0 : k) * h + i);
             }
             if (c > 0) { v = (double)s / ((double)FIX * (double)c); ++mine; }
             dst[i] = v;
@@ -310,6 +332,14 @@ __global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref,
     shift[2 * k + axis] = (double)best + delta;
 }
 
+int launch_mask_counts(const uint8_t* bad, int w, int h, int n, void* ws, cudaStream_t st)
+{
+    const EstimateWs e = carve_est(ws, w, h, n);
+    k_mask_counts<<<dim3(e.nbands), 256, 0, st>>>(bad, w, h, e);
+    MRED_LAUNCH_CHECK();
+    return MRED_OK;
+}
+
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
                     int32_t* ishift, double* shift, void* ws, int flags, cudaStream_t st)
 {
@@ -328,7 +358,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_correlate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
         attr_done = true;
     }
-    k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, bad ? 1 : 0, e);
+    k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, bad ? ((flags & EST_SHARED_COUNTS) ? 2 : 1) : 0, e);
     MRED_LAUNCH_CHECK();
     k_correlate<<<dim3(n, 2, CORR_Z), 256, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, e, ishift, shift);
     MRED_LAUNCH_CHECK();

@@ -336,12 +336,12 @@ def _chain_check(grp, max_lag, mode, full_size=False):
     return e
 
 
-def test_reduce_fused_profiles_ragged_matches_unfused_route():
-    """Without a bad-pixel mask mred_reduce sums the marginal profiles inside the calibrate kernel (k_calibrate_prof,
-    128 x 16 tiles, 4 frames per block); with a mask it runs k_calibrate + k_profiles.  On a geometry with odd
-    W, odd x0, w % 4 != 0 and ragged tiles (183 x 71, 6 frames = 4 + 2) the two routes must give the same
-    integer shifts, the same sub-pixel shifts to 1e-6 px and the same co-add; an all-zero mask
-    changes nothing in the definition (O4), so the oracle chain is the reference for both."""
+def test_reduce_fused_profiles_ragged_masked_and_unmasked():
+    """mred_reduce sums the marginal profiles inside the calibrate kernel (k_calibrate_prof, 128 x 16 tiles, 4 frames
+    per block); with a bad-pixel mask the same kernel leaves masked pixels out and k_mask_counts supplies the counts.
+    On a geometry with odd W, odd x0, w % 4 != 0 and ragged tiles (183 x 71, 6 frames = 4 + 2) both variants must
+    give the oracle's integer shifts, and the same sub-pixel shifts (to 1e-6 px) and co-add as each other: an
+    all-zero mask changes nothing in the definition (O4), so the oracle chain is the reference for both."""
     grp = synth.make_group(3, geom=GEOMS["ragged"], stars=25, S=5.0, n_sci=6, n_master=3)
     g, n = grp.geom, grp.sci.shape[0]
     m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
