@@ -40,6 +40,7 @@ extern "C" {
 
 #define MRED_MAX_STACK 255
 #define MRED_MAX_LAG 256
+#define MRED_MAX_PROFILE 4096 /* longest row / column mred_estimate_shifts and mred_reduce* accept */
 
 typedef struct {
     int32_t W, H;         /* raw frame size, x fastest (1074 x 1024 incl. overscan)   */
@@ -91,8 +92,8 @@ int mred_build_masters(const mred_geom *geom, const uint16_t *bias, int nb, cons
  *     out_k = (raw_k - L_k - MB - dark_scale * MD) / MF   on the image rectangle;  MF <= 0 or
  *     non-finite -> 0.   dark_scale = t_sci / t_dark.
  * raw: uint16 [n][H][W]; out: float32 [n][h][w]; level_out: float64 [n] (device, nullable)
- * receives L_k.  n >= 1 (no upper bound other than memory).  ws holds ceil(H/256) partial overscan
- * sums per frame (mred_workspace_bytes).
+ * receives L_k.  1 <= n <= 524 280 (8 x 65535; MRED_EINVAL beyond).  ws holds ceil(H/256)
+ * partial overscan sums per frame (mred_workspace_bytes).
  */
 int mred_calibrate(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
                    const float *MD, const float *MF, float *out, double *level_out, void *ws, size_t ws_bytes,
@@ -106,6 +107,7 @@ int mred_calibrate(const mred_geom *geom, const uint16_t *raw, int n, float dark
  * reference: a source at (x, y) in the reference sits at (x+dx, y+dy) in frame k.
  * frames: float32 [n][h][w]; badmask: uint8 [h][w], nullable; ishift: int32 [n][2] (ix, iy);
  * shift: float64 [n][2] (dx, dy); both device.  0 <= max_lag <= MRED_MAX_LAG, max_lag < min(w,h).
+ * w, h <= MRED_MAX_PROFILE (a whole profile is sorted in shared memory); MRED_EINVAL beyond.
  */
 int mred_estimate_shifts(const float *frames, int n, int w, int h, int ref_index, int max_lag,
                          const uint8_t *badmask, int32_t *ishift, double *shift, void *ws, size_t ws_bytes,
@@ -145,7 +147,8 @@ int mred_coadd(const float *stack, int n, int w, int h, const int32_t *footprint
  * The marginal profiles of estimate_shifts are summed inside the calibrate kernel (same definition,
  * DESIGN.md O4, masked pixels left out; the calibrated stack is not read a second time).
  * raw: uint16 [n][H][W].  shift_out: float64 [n][2] device (nullable) receives (dx, dy);
- * footprint_out: int32 [n][4] device (nullable).  Other arguments as in the single calls.
+ * footprint_out: int32 [n][4] device (nullable).  Other arguments as in the single calls; in particular
+ * 4 <= w, h <= MRED_MAX_PROFILE and n <= MRED_MAX_STACK.
  */
 int mred_reduce(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
                 const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
@@ -175,6 +178,13 @@ int mred_reduce_host(const mred_geom *geom, const uint16_t *raw_host, int n, flo
                      const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
                      float fill, const mred_comb_opts *opts, float *out_host, uint16_t *count_host,
                      double *shift_host, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * Where mred_reduce / mred_reduce_staged leave their two intermediate stacks inside `ws` (byte offsets from ws):
+ * the calibrated stack (O3) and the registered stack (O5), both float32 [n][h][w].  They stay valid
+ * until ws is used again.  For inspection and stage-by-stage checks; MRED_EINVAL on a null pointer or bad geometry.
+ */
+int mred_reduce_workspace_views(const mred_geom *geom, int n, size_t *calibrated_offset, size_t *registered_offset);
 
 /* Scratch size for one call (call = mred_call).  geom may be NULL for the calls that take w, h
  * directly, in which case pass them through a mred_geom with only w, h set. */

@@ -18,7 +18,8 @@
  *   orc_level           P1  constant frame -> level exactly
  *   orc_build_masters   P3  identical frames -> that frame; flat = c*pattern -> pattern/<pattern>; P11 brute force
  *   orc_calibrate       P1/P2 closed forms (uniform flat identity, bias-only -> 0, synthetic inverse)
- *   orc_estimate_shifts P7  injected integer shift recovered exactly; self -> (0,0); constant -> 0
+ *   orc_estimate_shifts P7  injected integer shift recovered exactly; self -> (0,0); constant -> 0;
+ *                           exact two-spike ties pin the argmax rule O4(iv) (smaller |l|, then smaller l)
  *   orc_resample        P4  paper's B-spline-basis image vs analytic shift;
  *                       P5  SciPy natural CubicSpline, identity, integer shift, composition;
  *                       P6  round-trip magnitude vs the paper's printed 1e-2..1e-1 (L162, L225); P12 footprint

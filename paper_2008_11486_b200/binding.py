@@ -20,6 +20,7 @@ MAX_STACK = 255
 
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
            "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
+           "mred_reduce_workspace_views",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -77,6 +78,13 @@ def _dev(t, dtype, name):
     return C.c_void_p(t.data_ptr())
 
 
+def _shape(t, shape, name):
+    """Every tensor is checked against the geometry and frame count before the C ABI sees its pointer: the library
+    trusts sizes, so a mismatched tensor would be read or written out of bounds."""
+    if t is not None and tuple(t.shape) != tuple(shape):
+        raise MredError("%s has shape %s, expected %s" % (name, tuple(t.shape), tuple(shape)))
+
+
 def _stream(stream):
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
@@ -107,7 +115,11 @@ def build_masters(g, bias, dark, t_dark, flat, t_flat, mode=MEDIAN, ksigma=3.0, 
     """include/mred.h: mred_build_masters.  Returns (MB, MD, MF) float32 [h][w] CUDA tensors."""
     gg = geom(g)
     dev = bias.device
-    MB, MD, MF = out if out is not None else (torch.empty((gg.h, gg.w), dtype=torch.float32, device=dev) for _ in range(3))
+    MB, MD, MF = out if out is not None else [torch.empty((gg.h, gg.w), dtype=torch.float32, device=dev) for _ in range(3)]
+    for t, nm in ((bias, "bias"), (dark, "dark"), (flat, "flat")):
+        _shape(t, (t.shape[0], gg.H, gg.W), nm)
+    for t, nm in ((MB, "MB"), (MD, "MD"), (MF, "MF")):
+        _shape(t, (gg.h, gg.w), nm)
     nmax = max(bias.shape[0], dark.shape[0], flat.shape[0])
     ws = _ws(ws, workspace_bytes(CALL_BUILD_MASTERS, gg, nmax), dev)
     o = _opts(mode, ksigma, max_iter)
@@ -130,6 +142,11 @@ def calibrate(g, raw, dark_scale, MB, MD, MF, out=None, level_out=None, ws=None,
         out = torch.empty((n, gg.h, gg.w), dtype=torch.float32, device=dev)
     if level_out is None:
         level_out = torch.empty(n, dtype=torch.float64, device=dev)
+    _shape(raw, (n, gg.H, gg.W), "raw")
+    for t, nm in ((MB, "MB"), (MD, "MD"), (MF, "MF")):
+        _shape(t, (gg.h, gg.w), nm)
+    _shape(out, (n, gg.h, gg.w), "out")
+    _shape(level_out, (n,), "level_out")
     ws = _ws(ws, workspace_bytes(CALL_CALIBRATE, gg, n), dev)
     rc = lib().mred_calibrate(C.byref(gg), _dev(raw, torch.uint16, "raw"), C.c_int(n), C.c_float(dark_scale),
                               _dev(MB, torch.float32, "MB"), _dev(MD, torch.float32, "MD"),
@@ -146,6 +163,7 @@ def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stre
     dev = frames.device
     ish = torch.empty((n, 2), dtype=torch.int32, device=dev)
     sh = torch.empty((n, 2), dtype=torch.float64, device=dev)
+    _shape(badmask, (h, w), "badmask")
     gg = Geom(0, 0, 0, 0, 0, 0, w, h)
     ws = _ws(ws, workspace_bytes(CALL_ESTIMATE_SHIFTS, gg, n), dev)
     rc = lib().mred_estimate_shifts(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
@@ -170,6 +188,7 @@ def resample(frames, sx, sy, fill=0.0, out=None, ws=None, stream=None):
     sy = np.ascontiguousarray(np.broadcast_to(np.asarray(sy, np.float64), (n,)))
     if out is None:
         out = torch.empty_like(frames)
+    _shape(out, (n, h, w), "out")
     fp = np.zeros((n, 4), np.int32)
     rc = lib().mred_resample(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
                              sx.ctypes.data_as(C.c_void_p), sy.ctypes.data_as(C.c_void_p), C.c_float(fill),
@@ -225,11 +244,37 @@ class ReducePlan:
             self.shift = torch.empty((n, 2), dtype=torch.float64, device=dev)
             self.footprint = torch.empty((n, 4), dtype=torch.int32, device=dev)
 
+    def _view(self, which):
+        """float32 [n][h][w] view of the calibrated (0) / registered (1) stack mred_reduce left in the workspace
+        (mred_reduce_workspace_views); device plans only, valid until the plan is used again."""
+        if self.host:
+            raise MredError("workspace views exist for device plans only")
+        offs = (C.c_size_t(0), C.c_size_t(0))
+        _check(lib().mred_reduce_workspace_views(C.byref(self.g), C.c_int(self.n), C.byref(offs[0]), C.byref(offs[1])),
+               "mred_reduce_workspace_views")
+        nbytes = 4 * self.n * self.g.h * self.g.w
+        o = offs[which].value
+        return self.ws[o:o + nbytes].view(torch.float32).view(self.n, self.g.h, self.g.w)
+
+    def calibrated(self):
+        return self._view(0)
+
+    def registered(self):
+        return self._view(1)
+
+
+def _reduce_shapes(plan, raw, MB, MD, MF, badmask):
+    g = plan.g
+    _shape(raw, (plan.n, g.H, g.W), "raw")
+    for t, nm in ((MB, "MB"), (MD, "MD"), (MF, "MF"), (badmask, "badmask")):
+        _shape(t, (g.h, g.w), nm)
+
 
 def reduce(plan: ReducePlan, raw, dark_scale, MB, MD, MF, ref_index=0, max_lag=32, badmask=None, fill=0.0,
            mode=SIGCLIP, ksigma=3.0, max_iter=3, stream=None, events=None):
     """include/mred.h: mred_reduce / mred_reduce_staged (device-resident chained science path).  Results land
     in `plan`.  events: optional list of 5 torch.cuda.Event(enable_timing=True) recorded around the stages."""
+    _reduce_shapes(plan, raw, MB, MD, MF, badmask)
     o = _opts(mode, ksigma, max_iter)
     ev = C.c_void_p(None)
     if events is not None:
@@ -254,6 +299,9 @@ def reduce_host(plan: ReducePlan, raw_host, dark_scale, MB, MD, MF, ref_index=0,
     and shifts come back in plan.out / plan.count / plan.shift (pinned host tensors)."""
     if raw_host.is_cuda or raw_host.dtype != torch.uint16 or not raw_host.is_contiguous():
         raise MredError("raw_host must be a contiguous CPU uint16 tensor")
+    if not plan.host:
+        raise MredError("reduce_host needs a ReducePlan(host=True)")
+    _reduce_shapes(plan, raw_host, MB, MD, MF, badmask)
     o = _opts(mode, ksigma, max_iter)
     rc = lib().mred_reduce_host(C.byref(plan.g), C.c_void_p(raw_host.data_ptr()), C.c_int(plan.n),
                                 C.c_float(dark_scale), _dev(MB, torch.float32, "MB"), _dev(MD, torch.float32, "MD"),

@@ -10,6 +10,18 @@ namespace mred {
 static std::atomic<int> g_last_cuda_error{0};
 void set_cuda_error(cudaError_t e) { g_last_cuda_error.store((int)e); }
 
+int sm_count()
+{
+    static std::atomic<int> cached[64];
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    n = cached[dev].load(std::memory_order_relaxed);
+    if (n > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) return 148;
+    cached[dev].store(n, std::memory_order_relaxed);
+    return n;
+}
+
 static bool opts_ok(const mred_comb_opts* o)
 {
     if (!o) return false;
@@ -70,6 +82,23 @@ static HostWs carve_host(void* ws, const Geom& g, int n)
     r.reduce = take(carve_reduce(nullptr, g, n).bytes);
     r.bytes = (size_t)(p - static_cast<char*>(ws));
     return r;
+}
+
+// Everything mred_reduce* checks apart from the raw / out pointers (device for mred_reduce, host for
+// mred_reduce_host) and the workspace: shared so that mred_reduce_host can refuse a call before it enqueues anything.
+static int reduce_args_ok(const mred_geom* geom, int n, const float* MB, const float* MD, const float* MF, int ref_index,
+                          int max_lag, const uint8_t* badmask, const mred_comb_opts* opts, const uint16_t* count,
+                          const uint32_t* rejmask, const double* shift_out, const int32_t* footprint_out)
+{
+    if (!geom_ok(geom) || !MB || !MD || !MF || !opts_ok(opts)) return MRED_EINVAL;
+    if (n < 1 || n > MRED_MAX_STACK || geom->w < 4 || geom->h < 4 || geom->w > MRED_MAX_PROFILE || geom->h > MRED_MAX_PROFILE)
+        return MRED_EINVAL;
+    if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= geom->w || max_lag >= geom->h)
+        return MRED_EINVAL;
+    if (!aligned16(MB) || !aligned16(MD) || !aligned16(MF) || (count && !aligned16(count)) || (rejmask && !aligned16(rejmask)) ||
+        (badmask && !aligned16(badmask)) || (shift_out && !aligned16(shift_out)) || (footprint_out && !aligned16(footprint_out)))
+        return MRED_EALIGN;
+    return MRED_OK;
 }
 
 }  // namespace mred
@@ -153,7 +182,7 @@ int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index
                          void* stream)
 {
     if (!frames || !ishift || !shift || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1) return MRED_EINVAL;
-    if (w > 4096 || h > 4096) return MRED_EINVAL;   // profile length held in shared memory
+    if (w > MRED_MAX_PROFILE || h > MRED_MAX_PROFILE) return MRED_EINVAL;   // a whole profile is sorted in shared memory
     if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= w || max_lag >= h)
         return MRED_EINVAL;
     if (!aligned16(frames) || !aligned16(ishift) || !aligned16(shift) || (badmask && !aligned16(badmask)))
@@ -193,24 +222,29 @@ int mred_coadd(const float* stack, int n, int w, int h, const int32_t* footprint
                         static_cast<cudaStream_t>(stream));
 }
 
+int mred_reduce_workspace_views(const mred_geom* geom, int n, size_t* calibrated_offset, size_t* registered_offset)
+{
+    if (!geom_ok(geom) || n < 1 || n > MRED_MAX_STACK || !calibrated_offset || !registered_offset) return MRED_EINVAL;
+    char* base = nullptr;
+    const ReduceWs r = carve_reduce(base, to_geom(geom), n);
+    *calibrated_offset = (size_t)(reinterpret_cast<char*>(r.cal) - base);
+    *registered_offset = (size_t)(reinterpret_cast<char*>(r.reg) - base);
+    return MRED_OK;
+}
+
 int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
                        const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
                        const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
                        int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream, void* const* events)
 {
-    if (!geom_ok(geom) || !raw || !MB || !MD || !MF || !out || !opts_ok(opts)) return MRED_EINVAL;
-    if (n < 1 || n > MRED_MAX_STACK || geom->w < 4 || geom->h < 4 || geom->w > 4096 || geom->h > 4096) return MRED_EINVAL;
-    if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= geom->w || max_lag >= geom->h)
-        return MRED_EINVAL;
-    if (!aligned16(raw) || !aligned16(MB) || !aligned16(MD) || !aligned16(MF) || !aligned16(out) ||
-        (count && !aligned16(count)) || (rejmask && !aligned16(rejmask)) || (badmask && !aligned16(badmask)) ||
-        (shift_out && !aligned16(shift_out)) || (footprint_out && !aligned16(footprint_out)))
-        return MRED_EALIGN;
+    if (!raw || !out) return MRED_EINVAL;
+    if (!aligned16(raw) || !aligned16(out)) return MRED_EALIGN;
+    int rc = reduce_args_ok(geom, n, MB, MD, MF, ref_index, max_lag, badmask, opts, count, rejmask, shift_out, footprint_out);
+    if (rc) return rc;
     const Geom g = to_geom(geom);
     if (!ws || !aligned16(ws) || ws_bytes < carve_reduce(nullptr, g, n).bytes) return MRED_EWORKSPACE;
     const ReduceWs r = carve_reduce(ws, g, n);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    int rc;
 #define MRED_STAGE_EVENT(i) \
     do { if (events && events[i]) MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[i]), st)); } while (0)
     MRED_STAGE_EVENT(0);
@@ -255,7 +289,10 @@ int mred_reduce_host(const mred_geom* geom, const uint16_t* raw_host, int n, flo
                      const mred_comb_opts* opts, float* out_host, uint16_t* count_host, double* shift_host, void* ws,
                      size_t ws_bytes, void* stream)
 {
-    if (!geom_ok(geom) || !raw_host || !out_host || n < 1 || n > MRED_MAX_STACK) return MRED_EINVAL;
+    if (!raw_host || !out_host) return MRED_EINVAL;
+    // every argument is checked before the first copy is enqueued (header: nothing is enqueued on EINVAL / EALIGN / EWORKSPACE)
+    int rc = reduce_args_ok(geom, n, MB, MD, MF, ref_index, max_lag, badmask, opts, nullptr, nullptr, nullptr, nullptr);
+    if (rc) return rc;
     const Geom g = to_geom(geom);
     if (!ws || !aligned16(ws) || ws_bytes < carve_host(nullptr, g, n).bytes) return MRED_EWORKSPACE;
     const HostWs hw = carve_host(ws, g, n);
@@ -263,9 +300,9 @@ int mred_reduce_host(const mred_geom* geom, const uint16_t* raw_host, int n, flo
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t np = (size_t)g.w * g.h;
     MRED_CUDA_TRY(cudaMemcpyAsync(hw.raw, raw_host, 2 * (size_t)g.W * g.H * n, cudaMemcpyHostToDevice, st));
-    int rc = mred_reduce(geom, hw.raw, n, dark_scale, MB, MD, MF, ref_index, max_lag, badmask, fill, opts, hw.out,
-                         count_host ? hw.count : nullptr, nullptr, r.shift, nullptr, hw.reduce,
-                         carve_reduce(nullptr, g, n).bytes, stream);
+    rc = mred_reduce(geom, hw.raw, n, dark_scale, MB, MD, MF, ref_index, max_lag, badmask, fill, opts, hw.out,
+                     count_host ? hw.count : nullptr, nullptr, r.shift, nullptr, hw.reduce,
+                     carve_reduce(nullptr, g, n).bytes, stream);
     if (rc) return rc;
     MRED_CUDA_TRY(cudaMemcpyAsync(out_host, hw.out, 4 * np, cudaMemcpyDeviceToHost, st));
     if (count_host) MRED_CUDA_TRY(cudaMemcpyAsync(count_host, hw.count, 2 * np, cudaMemcpyDeviceToHost, st));

@@ -14,18 +14,19 @@ namespace mred {
 // the consumers add the nos = ceil(H/256) partials (integers: exact in any order).
 // Side job for the chained path: the blocks also clear `zero` (the accumulators of the kernels that follow on the
 // same stream), which saves the memset nodes between the stages.
-// grid (nos, n), block 256: one thread per row of the overscan strip
+// grid (nos * n) (1-D, so the frame count is not bound by the 65535 of gridDim.y), block 256: one thread per row
+// of the overscan strip
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_frame_sums(const uint16_t* __restrict__ raw, Geom g, int n,
+__global__ void __launch_bounds__(256) k_frame_sums(const uint16_t* __restrict__ raw, Geom g, int n, int nos,
                                                     unsigned long long* __restrict__ os_part,
                                                     uint4* __restrict__ zero, size_t zero_n16)
 {
     __shared__ unsigned long long s_w[8];
-    const int k = blockIdx.y;
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.x / nos, c = blockIdx.x - k * nos;
+    const int r = c * blockDim.x + threadIdx.x;
     if (zero) {
-        const size_t tid = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
-        const size_t nth = (size_t)gridDim.x * gridDim.y * blockDim.x;
+        const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+        const size_t nth = (size_t)gridDim.x * blockDim.x;
         for (size_t i = tid; i < zero_n16; i += nth) zero[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     unsigned long long s = 0;
@@ -36,7 +37,7 @@ __global__ void __launch_bounds__(256) k_frame_sums(const uint16_t* __restrict__
     if (threadIdx.x == 0) {
         unsigned long long t = 0;
         for (int i = 0; i < 8; ++i) t += s_w[i];
-        os_part[(size_t)k * gridDim.x + blockIdx.x] = t;
+        os_part[blockIdx.x] = t;          // = os_part[k * nos + c]
     }
 }
 
@@ -45,8 +46,8 @@ int frame_sums_parts(const Geom& g) { return (g.H + 255) / 256; }
 int launch_frame_sums(const uint16_t* raw, const Geom& g, int n, unsigned long long* os_part, void* zero,
                       size_t zero_bytes, cudaStream_t st)
 {
-    dim3 grid(frame_sums_parts(g), n);
-    k_frame_sums<<<grid, 256, 0, st>>>(raw, g, n, os_part, static_cast<uint4*>(zero), zero ? zero_bytes / 16 : 0);
+    const int nos = frame_sums_parts(g);
+    k_frame_sums<<<dim3((unsigned)(nos * n)), 256, 0, st>>>(raw, g, n, nos, os_part, static_cast<uint4*>(zero), zero ? zero_bytes / 16 : 0);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
@@ -325,6 +326,7 @@ int launch_calibrate(const uint16_t* raw, const Geom& g, int n, float dark_scale
     const int w4 = (g.w + 3) / 4;
     const long long groups = (long long)g.h * w4;
     const int fc = chunk_frames(n);
+    if ((n + fc - 1) / fc > 65535) return MRED_EINVAL;          // gridDim.y; n <= 524 280 (include/mred.h)
     dim3 grid((unsigned)((groups + 255) / 256), (unsigned)((n + fc - 1) / fc));
     const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
     k_calibrate<<<grid, 256, 0, st>>>(raw, g, n, fc, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), level_out, vec_ok);

@@ -1,6 +1,7 @@
 // common.cuh -- shared device helpers and host-side checks for libmred (sm_100a only).
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <stdint.h>
 #include <stddef.h>
 #include "../../include/mred.h"
@@ -31,6 +32,19 @@ inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 void set_cuda_error(cudaError_t e);   // api.cu
+int sm_count();                       // api.cu: multiprocessors of the current device (cached per device)
+
+// One-time, per-DEVICE setup (function attributes such as the dynamic shared-memory opt-in belong to the device's
+// context, not to the process): done[dev] is set once the attributes have been applied on that device.
+struct PerDeviceOnce {
+    std::atomic<unsigned char> done[64];
+    bool pending(int& dev)
+    {
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { dev = -1; return true; }   // unknown: set every time
+        return done[dev].load(std::memory_order_acquire) == 0;
+    }
+    void mark(int dev) { if (dev >= 0) done[dev].store(1, std::memory_order_release); }
+};
 
 #define MRED_CUDA_TRY(expr)                                   \
     do {                                                      \

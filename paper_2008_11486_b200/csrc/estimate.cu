@@ -16,7 +16,7 @@ namespace mred {
 constexpr int PROF_BR = 32;        // rows per band
 constexpr int RIF = 4;             // rows in flight per thread in k_profiles
 constexpr float FIX = PROF_FIX;    // fixed-point scale of the profile sums (common.cuh)
-constexpr int PROF_MAXLEN = 4096;  // longest profile the finalize kernel holds in shared memory
+constexpr int PROF_MAXLEN = MRED_MAX_PROFILE;  // longest profile the finalize kernel holds in shared memory
 
 struct EstimateWs {
     long long* colpart;  // [n][w]   fixed-point column sums (value * FIX), accumulated with integer atomics by the bands
@@ -352,11 +352,12 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     }
     int P = 1;
     while (P < (w > h ? w : h)) P <<= 1;
-    static bool attr_done = false;   // idempotent
-    if (!attr_done) {
+    static PerDeviceOnce once;
+    int dev;
+    if (once.pending(dev)) {
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_finalize, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_correlate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
-        attr_done = true;
+        once.mark(dev);
     }
     k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, bad ? ((flags & EST_SHARED_COUNTS) ? 2 : 1) : 0, e);
     MRED_LAUNCH_CHECK();

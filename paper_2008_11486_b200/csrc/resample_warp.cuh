@@ -581,10 +581,10 @@ __global__ void k_ypass4(const float* __restrict__ T, int n, int w, int h, const
                          const double* __restrict__ dshift, float fill, float* __restrict__ out, int4* __restrict__ fp_dev,
                          int BH);
 
-// band height for the kernels that carry y state: enough warps for 148 SMs x 8, no band under 64 rows
+// band height for the kernels that carry y state: enough warps for every SM x 8, no band under 64 rows
 static int band_rows(long long cols, int h, int min_rows = 64, int warps_per_sm = 8)
 {
-    long long bands = (148 * warps_per_sm + cols - 1) / cols;
+    long long bands = ((long long)sm_count() * warps_per_sm + cols - 1) / cols;
     const long long maxb = (h + min_rows - 1) / min_rows;
     if (bands > maxb) bands = maxb;
     if (bands < 1) bands = 1;
@@ -607,13 +607,14 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
         for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
     const int vec = (w % 4 == 0) ? 1 : 0;
     const size_t smem = (size_t)NRING * RB * WARPCOLS * sizeof(float);
-    static bool attr_done = false;   // idempotent: the same value every time, so a race is harmless
-    if (!attr_done) {
+    static PerDeviceOnce once;
+    int dev;
+    if (once.pending(dev)) {
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        attr_done = true;
+        once.mark(dev);
     }
     int4* fpd = reinterpret_cast<int4*>(fp_dev);
     const size_t need = resample_ws_bytes(w, h, n);
@@ -622,7 +623,8 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
         // neither kernel carries the other's state, so both run with far more parallel work items
         float* tmp = static_cast<float*>(ws);
         const int sx1 = (w + ModeGeom<1>::OUTC - 1) / ModeGeom<1>::OUTC;
-        int BH1 = (int)(((long long)h * sx1 * n + 148 * 16 - 1) / (148 * 16));     // one wave of 16 warps per SM
+        const int slots1 = sm_count() * 16;
+        int BH1 = (int)(((long long)h * sx1 * n + slots1 - 1) / slots1);     // one wave of 16 warps per SM
         BH1 = (BH1 + 3) / 4 * 4;
         if (BH1 < 8) BH1 = 8;
         k_resample<1><<<dim3(sx1, (h + BH1 - 1) / BH1, n), 32, 0, st>>>(in, n, w, h, hs, dshift_dev, fill, tmp, nullptr, BH1, vec);

@@ -1,7 +1,8 @@
 """GPU parity: every C-ABI call of libmred.so against the float64 CPU oracle, element by element on the
 same seeded inputs, stage-isolated (each GPU stage is fed the oracle's upstream output, Q19).
 Bar: bit-exact for integer outputs (away from clip-threshold ties, Q20); |d| <= 1e-3 + 1e-5 |ref| for
-float pixels (Q18); <= 1e-3 px for sub-pixel shifts.  Run on the B200 box with -m gpu."""
+float pixels (Q18; resample next to saturated spikes: Q18b, see assert_resample_close); <= 1e-3 px for sub-pixel
+shifts.  Run on the B200 box with -m gpu."""
 import numpy as np
 import pytest
 import torch
@@ -34,23 +35,68 @@ def host(t):
     return t.cpu().numpy()
 
 
-def assert_close(got, ref, what="", local=0):
-    """|d| <= 1e-3 + 1e-5 |ref| (Q18).  local = r > 0 (resample only, Q18b): |ref| is replaced by its
-    maximum over the (2r+1)^2 neighbourhood in the same plane, because the spline prefilter is a linear
-    operator that mixes neighbours with weights 0.268^d: float32 rounding is relative to the largest neighbour
-    (a 65535-ADU saturated pixel next to 1000-ADU sky), not to the value that remains after cancellation."""
+def assert_close(got, ref, what=""):
+    """The stated bar for float outputs, |d| <= 1e-3 + 1e-5 |ref| (Q18), on every element."""
     got = np.asarray(got, np.float64)
     ref = np.asarray(ref, np.float64)
     d = np.abs(got - ref)
-    mag = np.abs(ref)
-    if local:
-        from scipy.ndimage import maximum_filter
-        size = [1] * (ref.ndim - 2) + [2 * local + 1, 2 * local + 1]
-        mag = maximum_filter(mag, size=size, mode="nearest")
-    tol = 1e-3 + 1e-5 * mag
+    tol = 1e-3 + 1e-5 * np.abs(ref)
     bad = d > tol
     assert not bad.any(), "%s: %d of %d outside tolerance, max |d| = %g, max ratio = %g" % (
         what, bad.sum(), bad.size, d.max(), (d / tol).max())
+
+
+A_POLE = 2.0 - np.sqrt(3.0)      # |pole| of the cubic-spline prefilter: a coefficient feels a sample d away with weight a^d
+C_SPIKE = 1.0e-6                 # allowance per unit of neighbour magnitude (DESIGN.md Q18b): ~17 float32 roundings
+
+
+def spike_envelope(ref, reach=10):
+    """E(x, y) = max over (dx, dy) of |ref(x+dx, y+dy)| a^(|dx|+|dy|): the largest magnitude the separable spline
+    prefilter mixes into a pixel, each neighbour weighted by how much of it arrives there."""
+    e = np.abs(np.asarray(ref, np.float64))
+    for axis in (-1, -2):
+        out = e.copy()
+        for d in range(1, min(reach, e.shape[axis] - 1) + 1):
+            f = A_POLE ** d
+            lo = [slice(None)] * e.ndim
+            hi = [slice(None)] * e.ndim
+            lo[axis], hi[axis] = slice(None, -d), slice(d, None)
+            lo, hi = tuple(lo), tuple(hi)
+            np.maximum(out[lo], f * e[hi], out=out[lo])
+            np.maximum(out[hi], f * e[lo], out=out[hi])
+        e = out
+    return e
+
+
+def assert_resample_close(got, ref, what="", strict_everywhere=False):
+    """resample outputs (Q18 / Q18b).
+    * Every pixel without a much brighter neighbour ("quiet": E <= 2 |ref| + 100 ADU) must meet the stated bar
+      |d| <= 1e-3 + 1e-5 |ref|; with strict_everywhere (inputs without saturated spikes) every pixel must.
+    * Next to a spike float32 cannot do that: the prefilter is a linear operator that mixes a 65535-ADU neighbour into
+      a 1000-ADU pixel with weight a^d and every float32 rounding is relative to the LARGEST term, not to what is left
+      after cancellation.  There the bar is 1e-3 + 1e-5 |ref| + C_SPIKE * E, with E decaying as a^d away from the spike
+      (0.07 ADU beside a saturated pixel, 2e-3 four pixels away) -- not a flat 1e-5 of the neighbourhood maximum.
+    Returns (worst ratio to the stated bar, fraction of pixels that meet it, largest (|d| - bar) / E)."""
+    got = np.asarray(got, np.float64)
+    ref = np.asarray(ref, np.float64)
+    d = np.abs(got - ref)
+    bar = 1e-3 + 1e-5 * np.abs(ref)
+    env = spike_envelope(ref)
+    quiet = env <= 2.0 * np.abs(ref) + 100.0
+    ratio = d / bar
+    worst, frac_ok = float(ratio.max()), float((ratio <= 1.0).mean())
+    c_needed = float(((d - bar) / np.maximum(env, 1e-30)).max())
+    print("%s: max |d| %.3g ADU; stated bar: worst ratio %.3g, met by %.6f of the pixels; quiet pixels %.4f of all, "
+          "worst ratio there %.3g; c needed next to spikes %.3g" % (
+              what, d.max(), worst, frac_ok, quiet.mean(), ratio[quiet].max() if quiet.any() else 0.0, max(c_needed, 0.0)))
+    must = np.ones(ref.shape, bool) if strict_everywhere else quiet
+    bad = must & (ratio > 1.0)
+    assert not bad.any(), "%s: %d pixels outside the stated bar 1e-3 + 1e-5|ref| (worst ratio %g)" % (
+        what, bad.sum(), ratio[must].max())
+    bad = d > bar + C_SPIKE * env
+    assert not bad.any(), "%s: %d pixels outside 1e-3 + 1e-5|ref| + %g E next to spikes (c needed %g)" % (
+        what, bad.sum(), C_SPIKE, c_needed)
+    return worst, frac_ok, c_needed
 
 
 GEOMS = {
@@ -256,7 +302,7 @@ def test_resample_parity(shape):
     out, fp = mred.resample(dev(img), sx, sy, fill=-5.0)
     assert np.array_equal(fp, ref.footprint)                  # integer geometry bit-exact
     got = host(out)
-    assert_close(got, ref.out, "resample %s" % (shape,), local=4)
+    assert_resample_close(got, ref.out, "resample %s" % (shape,))
     for k, (a, b) in enumerate(SHIFTS):                        # integer shifts are exact copies
         if a == np.floor(a) and b == np.floor(b):
             assert np.array_equal(got[k], ref.out[k])
@@ -278,8 +324,8 @@ def test_resample_both_routes():
     two, fp2 = mred.resample(dev(img), sx, sy, fill=7.0)                 # workspace allocated by the binding
     one, fp1 = mred.resample(dev(img), sx, sy, fill=7.0, ws=False)       # fused kernel
     assert np.array_equal(fp1, ref.footprint) and np.array_equal(fp2, ref.footprint)
-    assert_close(host(two), ref.out, "resample two-kernel route", local=4)
-    assert_close(host(one), ref.out, "resample fused route", local=4)
+    assert_resample_close(host(two), ref.out, "resample two-kernel route")
+    assert_resample_close(host(one), ref.out, "resample fused route")
     for k, (a, b) in enumerate(SHIFTS):
         if a == np.floor(a) and b == np.floor(b):
             assert np.array_equal(host(two)[k], ref.out[k]) and np.array_equal(host(one)[k], ref.out[k])
@@ -302,38 +348,64 @@ def test_resample_bspline_image_matches_paper_precision(golden):
 
 
 # ------------------------------------------------------------------ chained path and full-size configs
-def _chain_check(grp, max_lag, mode, full_size=False):
-    """mred_reduce (device-chained) vs the oracle chain.  Integer outputs binding away from ties; shifts
-    within 1e-3 px; pixel maxima reported and bounded loosely (Q19: 1e-3 px near a bright star moves the
-    value by far more than the isolated tolerance)."""
+CHAIN_MARGIN = 0.05      # ADU: clip decisions closer than this to the threshold are not compared in the chained path (Q20)
+
+
+def _chain_check(grp, max_lag, mode, what, resample_frames=None):
+    """mred_reduce (the device-chained path bench.py times) against the oracle, stage by stage on the SAME upstream
+    data, so that every float comparison is at the stated bar (no loose percentile bound):
+      masters   mred_build_masters vs oracle (strict);
+      calibrate the calibrated stack mred_reduce left in its workspace (k_calibrate_prof) vs oracle.calibrate, both fed
+                the oracle's float32 masters: strict, every element;
+      shifts    within 1e-3 px of the oracle's, integer part bit-exact;
+      resample  the registered stack vs oracle.resample of the oracle's calibrated stack by the GPU's OWN shifts (the
+                1e-3 px the two estimates may differ by would otherwise move pixels next to a star by ~10 ADU, Q19);
+      coadd     value strict, count and rejection mask bit-exact away from clip-threshold ties (margin map).
+    resample_frames: indices of the frames whose registered planes are compared (None = all)."""
     g = grp.geom
-    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
-    c = oracle.calibrate(g, grp.sci, grp.t_sci / grp.t_dark, m.MB, m.MD, m.MF)
-    e = oracle.estimate_shifts(c.out, 0, max_lag, badmask=grp.badmask)
-    r = oracle.resample(c.out, -e.shift[:, 0], -e.shift[:, 1])
-    o = oracle.coadd(r.out, r.footprint, mode=mode)
     n = grp.sci.shape[0]
+    scale = grp.t_sci / grp.t_dark
+    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
     MB, MD, MF = mred.build_masters(g, dev(grp.bias), dev(grp.dark), grp.t_dark, dev(grp.flat), grp.t_flat)
-    assert_close(host(MB), m.MB, "MB")
-    assert_close(host(MF), m.MF, "MF")
+    for a, b, nm in ((MB, m.MB, "MB"), (MD, m.MD, "MD"), (MF, m.MF, "MF")):
+        assert_close(host(a), b, what + " " + nm)
+    del MB, MD, MF
+    c = oracle.calibrate(g, grp.sci, scale, m.MB, m.MD, m.MF)
+    e = oracle.estimate_shifts(c.out, 0, max_lag, badmask=grp.badmask)
     plan = mred.ReducePlan(g, n, want_mask=True)
     bad = dev(grp.badmask) if grp.badmask is not None else None
-    mred.reduce(plan, dev(grp.sci), grp.t_sci / grp.t_dark, MB, MD, MF, 0, max_lag, badmask=bad, mode=mode)
+    mred.reduce(plan, dev(grp.sci), scale, dev(m.MB), dev(m.MD), dev(m.MF), 0, max_lag, badmask=bad, mode=mode)
+    assert_close(host(plan.calibrated()), c.out, what + " calibrated stack (k_calibrate_prof)")
     sh = host(plan.shift)
     assert np.max(np.abs(sh - e.shift)) <= 1e-3, np.max(np.abs(sh - e.shift))
+    assert np.array_equal(np.floor(sh + 0.5).astype(np.int64), e.ishift.astype(np.int64))
+    assert np.all(sh[0] == 0.0)
+    r = oracle.resample(c.out, -sh[:, 0], -sh[:, 1])
     assert np.array_equal(host(plan.footprint), r.footprint)
+    reg = plan.registered()
+    idx = list(range(n)) if resample_frames is None else list(resample_frames)
+    spiked = grp.config == 4          # saturated stars, cosmic rays, hot columns
+    for k in idx:
+        assert_resample_close(host(reg[k]), r.out[k], "%s registered frame %d" % (what, k), strict_everywhere=not spiked)
+    o = oracle.coadd(r.out, r.footprint, mode=mode)
     got, cnt = host(plan.out), host(plan.count)
-    safe = np.ones(got.shape, bool) if mode != 2 else (o.margin >= 0.05)
-    assert np.array_equal(cnt[safe], o.count[safe])
-    if mode == 2:
-        mk = host(plan.mask)
-        for wd in range(mk.shape[0]):
-            assert np.array_equal(mk[wd][safe], o.rejmask[wd][safe])
-    d = np.abs(got.astype(np.float64) - o.out)[safe]
-    rel = d / (1e-3 + 1e-5 * np.abs(o.out[safe]))
-    print("chained: max |d| %.3g ADU, 99.9%% of pixels within %.3g x tolerance" % (d.max(), np.percentile(rel, 99.9)))
-    assert np.percentile(rel, 99) < 50.0
-    return e
+    safe = np.ones(got.shape, bool) if mode != 2 else (o.margin >= CHAIN_MARGIN)
+    print("%s: %.5f of the pixels within %.2f ADU of a clip tie (not compared)" % (what, (~safe).mean(), CHAIN_MARGIN))
+    assert (~safe).mean() < 0.02
+    assert np.array_equal(cnt[safe], o.count[safe]), "count differs on %d px" % (cnt[safe] != o.count[safe]).sum()
+    mk = host(plan.mask)
+    for wd in range(mk.shape[0]):
+        assert np.array_equal(mk[wd][safe], o.rejmask[wd][safe]), "rejection mask word %d" % wd
+    if spiked:
+        # the registered frames differ from the oracle's by up to C_SPIKE * E next to spikes; the co-add of the
+        # survivors inherits at most the largest of those differences
+        env = np.max(np.stack([spike_envelope(r.out[k]) for k in range(n)]), axis=0)
+        d = np.abs(got.astype(np.float64) - o.out)
+        tol = 1e-3 + 1e-5 * np.abs(o.out) + C_SPIKE * env
+        assert not (d > tol)[safe].any(), "co-add: %d px outside, worst ratio %g" % ((d > tol)[safe].sum(), (d / tol)[safe].max())
+    else:
+        assert_close(got[safe], o.out[safe], what + " co-add")
+    return e, plan
 
 
 def test_reduce_fused_profiles_ragged_masked_and_unmasked():
@@ -363,9 +435,11 @@ def test_reduce_fused_profiles_ragged_masked_and_unmasked():
 
 def test_reduce_chain_small():
     grp = synth.make_group(1, geom=synth.GEOM_SMALL, stars=30, S=6.0)
-    _chain_check(grp, 12, 0)
+    _chain_check(grp, 12, 0, "small config 1")
     grp = synth.make_group(4, geom=synth.GEOM_SMALL, stars=30, S=6.0, n_sci=24, n_master=4)
-    _chain_check(grp, 12, 2)
+    _chain_check(grp, 12, 2, "small config 4")
+    grp = synth.make_group(3, geom=GEOMS["ragged"], stars=25, S=5.0, n_sci=7, n_master=3)     # odd W, x0; w % 4 != 0
+    _chain_check(grp, 10, 2, "ragged config 3")
 
 
 def test_config1_full_size_stage_isolated():
@@ -389,7 +463,7 @@ def test_config1_full_size_stage_isolated():
     r = oracle.resample(c.out, -e.shift[:, 0], -e.shift[:, 1])
     reg, fp = mred.resample(dev(c.out), -e.shift[:, 0], -e.shift[:, 1])
     assert np.array_equal(fp, r.footprint)
-    assert_close(host(reg), r.out, "resample", local=4)
+    assert_resample_close(host(reg), r.out, "resample config 1", strict_everywhere=True)
     _compare_coadd(r.out, r.footprint, 0)
     _compare_coadd(r.out, r.footprint, 2)
 
@@ -398,9 +472,45 @@ def test_config2_group_full_size_chained():
     """BASELINE.json config 2 (the bench workload): one group at full size through mred_build_masters + mred_reduce,
     exactly the calls and launch configuration bench.py times (10 frames: two-kernel resample route, N = 10 buckets)."""
     grp = synth.make_group(2, 1)
-    e = _chain_check(grp, 32, 2)
+    e, _ = _chain_check(grp, 32, 2, "config 2")
     assert np.array_equal(np.rint(e.shift), np.rint(grp.shifts))          # diagnostic: integer part of the truth
     assert np.max(np.abs(e.shift - grp.shifts)) < 0.05
+
+
+def test_config3_group_full_size_chained():
+    """BASELINE.json config 3 (bench.py's default workload): one (telescope, band) group at full size, 60 science
+    frames with per-frame sky 500-3000 ADU and 20/20/20 masters, through mred_build_masters + mred_reduce exactly as
+    bench.py launches them (N = 60 co-add bucket, N = 20 master buckets, the resample route of a 251 MB stack)."""
+    grp = synth.make_group(3, 2)
+    e, _ = _chain_check(grp, 40, 2, "config 3")
+    assert np.array_equal(np.rint(e.shift), np.rint(grp.shifts))
+    assert np.max(np.abs(e.shift - grp.shifts)) < 0.05
+
+
+def test_config4_full_size_chained_with_badmask():
+    """BASELINE.json config 4 through mred_reduce with its real hot-column bad-pixel mask: 64 frames, cosmic rays,
+    saturated stars; the masked fused calibrate kernel, k_mask_counts, the shared counts in k_finalize, the 64-frame
+    co-add with a 2-word rejection mask.  Registered planes compared on a sample of frames."""
+    grp = synth.make_group(4)
+    assert grp.badmask is not None and grp.badmask.any()
+    e, _ = _chain_check(grp, 16, 2, "config 4", resample_frames=(1, 17, 40, 63))
+    assert np.max(np.abs(e.shift - grp.shifts)) < 0.5          # diagnostic (Q10: cosmic rays cost accuracy)
+
+
+def test_config5_large_format_chained():
+    """BASELINE.json config 5 geometry through mred_reduce: 10 frames of 4128 x 4096 (k_calibrate_prof on 4096-wide
+    tiles with masters beyond L2, the large-plane resample route, 4096 x 4096 co-add)."""
+    grp = synth.make_group(5, n_sci=10, n_master=3, stars=400)
+    e, _ = _chain_check(grp, 64, 2, "config 5 (10 frames)", resample_frames=(1, 9))
+    assert np.max(np.abs(e.shift - grp.shifts)) < 0.05
+
+
+def test_config5_coadd_100_frames_strip():
+    """The 100-frame co-add bucket of config 5 (k_coadd for N = 100, sigma-clip, 4-word mask) on a real strip of the
+    large plane: 100 x 64 x 4096 with footprints, against oracle.coadd."""
+    st, fp = _stack(100, 64, 4096, 555, hits=0.003)
+    _compare_coadd(st, fp, 2)
+    _compare_coadd(st, fp, 0)
 
 
 def test_config4_stress_coadd_full_size():
@@ -413,7 +523,7 @@ def test_config4_stress_coadd_full_size():
     reg, fp = mred.resample(dev(c.out), sx, sy)
     # resample parity on a sample of frames (the oracle takes ~0.1 s per frame)
     r = oracle.resample(c.out[:4], sx[:4], sy[:4])
-    assert_close(host(reg)[:4], r.out, "resample cfg4", local=4)
+    assert_resample_close(host(reg)[:4], r.out, "resample config 4")
     st = host(reg)
     _compare_coadd(st, fp, 2)
 
@@ -440,8 +550,8 @@ def test_config5_geometry_two_frames():
     two, fp2 = mred.resample(dev(c.out[1:]), sx[1:], sy[1:])
     one, fp1 = mred.resample(dev(c.out[1:]), sx[1:], sy[1:], ws=False)
     assert np.array_equal(fp1, r.footprint) and np.array_equal(fp2, r.footprint)
-    assert_close(host(two), r.out, "resample large, two kernels", local=4)
-    assert_close(host(one), r.out, "resample large, fused", local=4)
+    assert_resample_close(host(two), r.out, "resample large, with workspace", strict_everywhere=True)
+    assert_resample_close(host(one), r.out, "resample large, fused", strict_everywhere=True)
 
 
 def test_single_frame_stacks_and_zero_lag():
@@ -469,7 +579,76 @@ def test_single_frame_stacks_and_zero_lag():
     r = oracle.resample(c.out, [0.37], [-1.2])
     reg, fp = mred.resample(dev(c.out), [0.37], [-1.2])
     assert np.array_equal(fp, r.footprint)
-    assert_close(host(reg), r.out, "resample n=1", local=4)
+    assert_resample_close(host(reg), r.out, "resample n=1", strict_everywhere=True)
+
+
+# ------------------------------------------------------------------ the remaining parity findings of round 1
+def test_resample_stated_bar_without_spikes():
+    """The stated bar (1e-3 + 1e-5 |ref|) on EVERY pixel for inputs without saturated spikes: a noise field with Table 4's
+    background and RMS, and a star field like config 1 (peaks up to 20 000 ADU on 1000 ADU sky)."""
+    h, w = 300, 420
+    rng = np.random.default_rng(77)
+    n = len(SHIFTS)
+    noise = rng.normal(705.0, 23.741, size=(n, h, w)).astype(np.float32)
+    sx = np.array([s[0] for s in SHIFTS])
+    sy = np.array([s[1] for s in SHIFTS])
+    ref = oracle.resample(noise, sx, sy)
+    for ws in (None, False):                                   # both routes of mred_resample
+        out, _ = mred.resample(dev(noise), sx, sy, ws=ws)
+        assert_resample_close(host(out), ref.out, "noise field, ws=%s" % ws, strict_everywhere=True)
+    yy, xx = np.mgrid[0:h, 0:w]
+    stars = rng.normal(1000.0, 31.0, size=(h, w))
+    for _ in range(60):
+        x, y, a = rng.uniform(0, w), rng.uniform(0, h), np.exp(rng.uniform(np.log(200), np.log(20000)))
+        stars += a * np.exp(-0.5 * ((xx - x) ** 2 + (yy - y) ** 2) / 1.274 ** 2)
+    img = np.repeat(stars[None].astype(np.float32), n, axis=0)
+    ref = oracle.resample(img, sx, sy)
+    for ws in (None, False):
+        out, _ = mred.resample(dev(img), sx, sy, ws=ws)
+        assert_resample_close(host(out), ref.out, "star field, ws=%s" % ws, strict_everywhere=True)
+
+
+def test_reduce_host_matches_reduce():
+    """mred_reduce_host (host uint16 in, host float32 co-add out: the call behind bench.py's e2e figure) must return
+    bit for bit what mred_reduce returns on the same group: out, count and shifts."""
+    cases = [synth.make_group(1, geom=synth.GEOM_SMALL, stars=30, S=6.0),
+             synth.make_group(4, geom=synth.GEOM_SMALL, stars=30, S=6.0, n_sci=24, n_master=4),
+             synth.make_group(1)]                                                      # full size, 5 frames
+    for grp in cases:
+        g, n = grp.geom, grp.sci.shape[0]
+        mode = grp.coadd
+        MB, MD, MF = mred.build_masters(g, dev(grp.bias), dev(grp.dark), grp.t_dark, dev(grp.flat), grp.t_flat)
+        bad = dev(grp.badmask) if grp.badmask is not None else None
+        plan = mred.ReducePlan(g, n)
+        mred.reduce(plan, dev(grp.sci), 1.0, MB, MD, MF, 0, 12, badmask=bad, mode=mode)
+        hplan = mred.ReducePlan(g, n, host=True)
+        raw_host = torch.from_numpy(np.ascontiguousarray(grp.sci)).pin_memory()
+        mred.reduce_host(hplan, raw_host, 1.0, MB, MD, MF, 0, 12, badmask=bad, mode=mode)
+        torch.cuda.synchronize()
+        assert np.array_equal(hplan.out.numpy(), host(plan.out))
+        assert np.array_equal(hplan.count.numpy(), host(plan.count))
+        assert np.array_equal(hplan.shift.numpy(), host(plan.shift))
+        # and it refuses bad arguments before enqueuing anything (include/mred.h)
+        with pytest.raises(mred.MredError, match="invalid argument"):
+            mred.reduce_host(hplan, raw_host, 1.0, MB, MD, MF, n + 3, 12, badmask=bad, mode=mode)
+
+
+def test_estimate_shifts_tie_rule():
+    """O4(iv) on exact ties (the frames of the oracle pin test_p7_argmax_tie_rule): C(-5) == C(+2) -> +2,
+    C(-3) == C(+3) -> -3, C(-2) == C(+5) -> -2, C(-4) == C(+3) -> +3, sub-pixel part exactly 0; through the stand-alone
+    call (k_profiles) and through mred_reduce (profile sums of k_calibrate_prof)."""
+    from test_oracle_pins import tie_frames
+    fr = tie_frames()
+    e = oracle.estimate_shifts(fr, 0, 8)
+    ish, sh = mred.estimate_shifts(dev(fr), 0, 8)
+    assert host(ish).tolist() == [[0, 0], [2, -3], [-2, 3]] and np.array_equal(host(ish), e.ishift)
+    assert np.array_equal(host(sh), e.shift)
+    n, h, w = fr.shape
+    g = Geom(w, h, 0, 0, 0, 0, w, h)                           # no overscan: raw counts are the frames themselves
+    z, one = np.zeros((h, w), np.float32), np.ones((h, w), np.float32)
+    plan = mred.ReducePlan(g, n)
+    mred.reduce(plan, dev(fr.astype(np.uint16)), 1.0, dev(z), dev(z), dev(one), 0, 8, mode=1)
+    assert np.array_equal(host(plan.shift), e.shift)
 
 
 # ------------------------------------------------------------------ error behaviour

@@ -314,6 +314,41 @@ def test_p7_constant_image_and_badmask():
     assert tuple(e2.ishift[1]) == (a, b)
 
 
+def tie_frames():
+    """Frames whose median-subtracted profiles are exact small integers, so that the correlation of O4(iii) has EXACT
+    ties: along x the frame's profile holds two equal spikes 5 columns before and 2 after the reference spike
+    (C(-5) == C(+2)), along y two equal spikes 3 rows before and 3 after (C(-3) == C(+3)).  w, h are powers of two and
+    the values integers, so every mean, the median (the background level) and every product is exact in float32 and
+    float64 alike.  Frame 2 swaps the roles (spikes at -2 / +5 and again -3 / +3 with unequal |l| partners)."""
+    w, h = 64, 32
+    def frame(xs, ys):
+        px = np.zeros(w); py = np.zeros(h)
+        for x in xs: px[x] += 8.0
+        for y in ys: py[y] += 16.0
+        return (100.0 + px[None, :] + py[:, None]).astype(np.float32)
+    ref = frame([30], [15])
+    f1 = frame([30 - 5, 30 + 2], [15 - 3, 15 + 3])
+    f2 = frame([30 - 2, 30 + 5], [15 - 4, 15 + 3])
+    return np.stack([ref, f1, f2])
+
+
+def test_p7_argmax_tie_rule():
+    """O4(iv): ties of the correlation maximum go to the smaller |l|, then to the smaller l.  C(-5) == C(+2) -> +2;
+    C(-3) == C(+3) -> -3; C(-2) == C(+5) -> -2; C(-4) == C(+3) -> +3.  The parabola of an isolated spike has
+    C(l*-1) = C(l*+1) = 0, so the sub-pixel part is exactly 0."""
+    fr = tie_frames()
+    e = oracle.estimate_shifts(fr, 0, 8)
+    assert e.ishift.tolist() == [[0, 0], [2, -3], [-2, 3]]
+    assert np.array_equal(e.shift, e.ishift.astype(np.float64))
+    # the tie is real: moving one spike by a column breaks it the other way
+    fr2 = fr.copy()
+    fr2[1, :, 25] -= 1.0            # weaken the spike at lag -5: +2 wins on value alone; (was a tie before)
+    assert oracle.estimate_shifts(fr2, 0, 8).ishift[1, 0] == 2
+    fr2 = fr.copy()
+    fr2[1, :, 32] -= 1.0            # weaken the spike at lag +2: -5 wins although |l| is larger
+    assert oracle.estimate_shifts(fr2, 0, 8).ishift[1, 0] == -5
+
+
 def test_p7_subpixel_parabola_closed_form():
     """Profiles built so that the correlation around the peak is an exact parabola."""
     w, h = 64, 48
