@@ -6,6 +6,7 @@
 // N x 256 x 4 B in flight).  HBM roofline: N*4 B read + 4 B value + 2 B count (+ 4*ceil(N/32) B
 // mask) written per pixel.
 #include "combine.cuh"
+#include "coadd_stream.cuh"
 
 namespace mred {
 
@@ -230,6 +231,21 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
     const int4* fpd = reinterpret_cast<const int4*>(fp_dev);
     const float ks = o.ksigma;
     const int mi = o.max_iter;
+    if (o.mode != MRED_MEDIAN && np % 4 == 0) {
+        // mean / sigma-clipped mean: streaming pass + compacted clip pass on bulk-copy-staged tiles (coadd_stream.cuh);
+        // planes whose size is not a multiple of 4 pixels (tiles not 16-byte aligned) keep the register kernels below
+        static PerDeviceOnce once;
+        int dev;
+        if (once.pending(dev)) {
+            MRED_CUDA_TRY(cudaFuncSetAttribute(k_coadd_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, MRED_MAX_STACK * cs::TP * 4));
+            MRED_CUDA_TRY(cudaFuncSetAttribute(k_coadd_stream, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+            once.mark(dev);
+        }
+        k_coadd_stream<<<dim3((unsigned)((np + cs::TP - 1) / cs::TP)), cs::TP, (size_t)n * cs::TP * 4, st>>>(
+            stack, n, w, h, fpd, use_fp, local, o.mode == MRED_SIGCLIP ? 1 : 0, ks, mi, out, count, rejmask);
+        MRED_LAUNCH_CHECK();
+        return MRED_OK;
+    }
     if (n <= 128) {
         dim3 grid((unsigned)((np + 255) / 256));
 #define MRED_CO(N) launch_mode<N>(o.mode, grid, st, stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask)

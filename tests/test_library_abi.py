@@ -42,9 +42,9 @@ def test_host_only_calls(libpath):
     assert need >= 2 * 10 * 1024 * 1024 * 4
     assert m.reduce_host_workspace_bytes(g, 10) >= need + 10 * 1074 * 1024 * 2
     assert m.workspace_bytes(m.CALL_COADD, g, 10) == 0
-    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 10) == 10 * 1024 * 1024 * 4      # small stack: two-kernel route
-    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 60) == 60 * 1024 * 1024 * 4
-    assert m.workspace_bytes(m.CALL_RESAMPLE, (4128, 4096, 0, 32, 32, 0, 4096, 4096), 100) == 0   # large planes: fused kernel
+    assert m.workspace_bytes(m.CALL_RESAMPLE, g, 10) == 0      # 16-byte-aligned rows, >= 256 x 64: the tiled kernel, no scratch
+    assert m.workspace_bytes(m.CALL_RESAMPLE, (4128, 4096, 0, 32, 32, 0, 4096, 4096), 100) == 0
+    assert m.workspace_bytes(m.CALL_RESAMPLE, (0, 0, 0, 0, 0, 0, 192, 136), 12) == 12 * 192 * 136 * 4   # small planes: x kernel + y kernel
 
 
 def test_sass_is_sm100a(libpath):
