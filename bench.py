@@ -35,12 +35,13 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default: configs[1])")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5 (default 3: the largest 1074x1024 workload, stacks beyond L2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--streams", type=int, default=0, help="CUDA streams the groups are spread over (0 = one per group)")
     ap.add_argument("--no-graph", action="store_true", help="plain launches in the timed region instead of a CUDA graph replay")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the short runs of configs 2 and 5 reported under `extra`")
     return ap.parse_args()
 
 
@@ -60,8 +61,11 @@ def rank_group_ids(cfg, rank):
 def make_groups(cfg, rank):
     from concurrent.futures import ThreadPoolExecutor
     ids = rank_group_ids(cfg, rank)
+    cores = os.cpu_count() or 8
+    if len(ids) == 1:
+        return [synth.make_group(cfg, ids[0], workers=min(16, cores))]
     with ThreadPoolExecutor(max_workers=min(8, len(ids))) as ex:
-        return list(ex.map(lambda gid: synth.make_group(cfg, gid), ids))
+        return list(ex.map(lambda gid: synth.make_group(cfg, gid, workers=max(1, min(16, cores) // min(8, len(ids)))), ids))
 
 
 def max_over_ranks(value, device=None):
@@ -206,34 +210,40 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------
-KERNELS_PER_BUILD_MASTERS = 4    # k_master_sums, k_masters_bd, k_masters_f, k_mf_scale
-KERNELS_PER_REDUCE = 7           # k_frame_sums, k_calibrate, k_profiles, k_finalize, k_correlate, k_resample, k_coadd (+1: small stacks resample in two kernels); memset nodes not counted
-KERNELS_PER_REDUCE_FUSED = 6     # mred_reduce: k_calibrate_prof replaces k_calibrate + k_profiles (+1 with a bad-pixel mask: k_mask_counts)
+ALL_STAGES = ["build_masters"] + STAGES
 
 
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
-    from paper_2008_11486_b200 import binding as mred
+def kernels_per_group(mred, g, n, masked):
+    """Kernels this repo launches per group and step (memset nodes not counted): mred_build_masters = k_master_sums,
+    k_masters_bd, k_masters_f, k_mf_scale; mred_reduce = k_frame_sums, [k_mask_counts], k_calibrate_prof, k_finalize,
+    k_correlate, the resample kernel(s) (one tiled kernel, or x kernel + y kernel on small planes), the co-add kernel."""
+    resample = 2 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 1
+    return 4 + 4 + (1 if masked else 0) + resample + 1
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
-    torch.cuda.set_device(local)
-    devs = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=devs)
-    mred.lib()
-    cfg = args.config
+
+def stage_kernels(mred, g, n, mode):
+    tiled = g.w % 4 == 0 and g.w >= 256 and g.h >= 64
+    return {"build_masters": "k_masters_bd + k_masters_f (+ k_master_sums, k_mf_scale)",
+            "calibrate": "k_calibrate_prof (+ k_frame_sums)",
+            "estimate_shifts": "k_finalize, k_correlate (profile sums come from k_calibrate_prof)",
+            "resample": "k_resample_tile (TMA-staged, x + y fused)" if tiled else "k_resample<1> + k_ypass4 (x pass, y pass)",
+            "coadd": "k_coadd_stream (bulk-copy staged)" if mode != 0 and (g.w * g.h) % 4 == 0 else "k_coadd<N,MODE>"}
+
+
+def bench_config(cfg, args, steps, warmup, mred, torch, dist, devs, rank, world, local):
+    """The whole hot path on BASELINE.json config `cfg`: returns the timed figures (device time, max over ranks)."""
     sp = synth.CONFIGS[cfg]
     g = sp["geom"]
     n, nm, G = sp["n_sci"], sp["n_master"], sp["groups"]
     groups = make_groups(cfg, rank)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    host = [dict(bias=pin(gr.bias), dark=pin(gr.dark), flat=pin(gr.flat), sci=pin(gr.sci)) for gr in groups]
-    devg = [{k: v.to(devs) for k, v in h.items()} for h in host]
+    want_host = not args.no_e2e and cfg == args.config
+    host = [dict(bias=pin(gr.bias), dark=pin(gr.dark), flat=pin(gr.flat), sci=pin(gr.sci)) for gr in groups] if want_host else None
+    if want_host:
+        devg = [{k: v.to(devs) for k, v in h.items()} for h in host]
+    else:
+        devg = [{k: torch.from_numpy(np.ascontiguousarray(getattr(gr, k))).to(devs) for k in ("bias", "dark", "flat", "sci")}
+                for gr in groups]
     bad = [torch.from_numpy(gr.badmask).to(devs) if gr.badmask is not None else None for gr in groups]
     words = (n + 31) // 32 if sp["stress"] else 0
     plans = [mred.ReducePlan(g, n, device=devs, want_mask=bool(words)) for _ in range(G)]
@@ -242,7 +252,9 @@ def run_ours(args):
     mode = groups[0].coadd
     lag = MAX_LAG[cfg]
     scale = groups[0].t_sci / groups[0].t_dark
-    nstage = len(STAGES)
+    t_dark, t_flat = groups[0].t_dark, groups[0].t_flat
+    truth = [gr.shifts for gr in groups]
+    del groups
 
     # groups are independent: each runs on its own stream, so that the small per-group kernels of different
     # groups overlap; a step starts and ends on the current stream (fork / join by events)
@@ -264,7 +276,7 @@ def run_ours(args):
             with torch.cuda.stream(st) if st is not None else contextlib.nullcontext():
                 if ev_m is not None:
                     ev_m[gi][0].record()
-                MB, MD, MF = mred.build_masters(g, d["bias"], d["dark"], groups[gi].t_dark, d["flat"], groups[gi].t_flat,
+                MB, MD, MF = mred.build_masters(g, d["bias"], d["dark"], t_dark, d["flat"], t_flat,
                                                 mode=mred.MEDIAN, ws=mwss[gi % len(streams)], out=masters_out[gi])
                 masters_out[gi] = (MB, MD, MF)
                 if ev_m is not None:
@@ -286,12 +298,13 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         flush.fill_(1)
         step(None, None)
     barrier()
-    # the step enqueues ~15 small kernels per group: capture it once in a CUDA graph and replay it in the timed
-    # region (launch-bound inner loop); the event-instrumented passes below run the same step without the graph
+    # the step enqueues ~11 kernels per group: capture it once in a CUDA graph and replay it in the timed
+    # region (launch-bound inner loop at the small configs); the event-instrumented passes below run the same step
+    # without the graph
     graph = None
     if not args.no_graph:
         try:
@@ -310,7 +323,7 @@ def run_ours(args):
     barrier()
     wall0 = time.perf_counter()
     step_ev, stage_ev = [], []
-    for _ in range(args.steps):
+    for _ in range(steps):
         flush.fill_(1)                       # cold L2 before every timed step (not inside the step's events)
         s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         evm, evs = new_events()
@@ -327,97 +340,69 @@ def run_ours(args):
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     if graph is not None:                                  # per-stage events: same step, same streams, plain launches
-        for _ in range(max(3, args.steps)):
+        for _ in range(max(3, steps)):
             flush.fill_(1)
             evm, evs = new_events()
             step(evm, evs)
             stage_ev.append((evm, evs))
         barrier()
     step_ms = [a.elapsed_time(b) for a, b in step_ev]
-    total_ms = float(sum(step_ms))
-    total_ms = max_over_ranks(total_ms, devs)
+    total_ms = max_over_ranks(float(sum(step_ms)), devs)
     frames_per_step = G * n * world
-    value = frames_per_step * args.steps / (total_ms * 1e-3)
+    value = frames_per_step * steps / (total_ms * 1e-3)
 
-    # per-stage device times inside the timed region (average per call = per group)
-    fused = True                     # mred_reduce always sums the profiles inside the calibrate kernel
-    masked = any(b is not None for b in bad)
-    sb = stage_bytes(g, n, nm, words, fused_profiles=fused)
-    st_ms = {k: [] for k in ["build_masters"] + STAGES}
-    for evm, evs in stage_ev:
-        for gi in range(G):
-            st_ms["build_masters"].append(evm[gi][0].elapsed_time(evm[gi][1]))
-            for i, nmst in enumerate(STAGES):
-                st_ms[nmst].append(evs[gi][i].elapsed_time(evs[gi][i + 1]))
+    def collect(evlist):
+        ms = {k: [] for k in ALL_STAGES}
+        for evm, evs in evlist:
+            for gi in range(G):
+                ms["build_masters"].append(evm[gi][0].elapsed_time(evm[gi][1]))
+                for i, nmst in enumerate(STAGES):
+                    ms[nmst].append(evs[gi][i].elapsed_time(evs[gi][i + 1]))
+        return ms
+
+    st_ms = collect(stage_ev)
     # the same step once more with every group on ONE stream: per-stage durations without overlap between groups
     iso_ms = None
     if len(streams) > 1:
         keep, streams[:] = list(streams), [None]
         iso_ev = []
-        for _ in range(max(3, args.steps)):
+        for _ in range(max(3, steps)):
             flush.fill_(1)
             evm, evs = new_events()
             step(evm, evs)
             iso_ev.append((evm, evs))
         barrier()
         streams[:] = keep
-        iso_ms = {k: [] for k in ["build_masters"] + STAGES}
-        for evm, evs in iso_ev:
-            for gi in range(G):
-                iso_ms["build_masters"].append(evm[gi][0].elapsed_time(evm[gi][1]))
-                for i, nmst in enumerate(STAGES):
-                    iso_ms[nmst].append(evs[gi][i].elapsed_time(evs[gi][i + 1]))
+        iso_ms = collect(iso_ev)
     peaks = {}
     pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk_path):
         peaks = json.load(open(pk_path))
     peak, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json)") if "hbm_gbs" in peaks else (6650.0, "fallback")
-    stages = {}
-    for k, v in st_ms.items():
-        ms = float(np.mean(v))
-        gbs = sb[k] / (ms * 1e-3) / 1e9
-        stages[k] = {"ms_per_call": round(ms, 5), "algorithmic_MB": round(sb[k] / 1e6, 3), "GBps": round(gbs, 1),
-                     "frac": round(gbs / peak, 4)}
-    stages_iso = None
-    if iso_ms is not None:
-        stages_iso = {}
-        for k, v in iso_ms.items():
+    sb = stage_bytes(g, n, nm, words, fused_profiles=True)   # mred_reduce sums the profiles inside the calibrate kernel
+
+    def table(ms_by_stage):
+        out = {}
+        for k, v in ms_by_stage.items():
             ms = float(np.mean(v))
             gbs = sb[k] / (ms * 1e-3) / 1e9
-            stages_iso[k] = {"ms_per_call": round(ms, 5), "GBps": round(gbs, 1), "frac": round(gbs / peak, 4)}
-    # dominant stage of the science path; its duration is taken without overlap from other groups when the step ran
-    # on several streams (an event interval on one stream then also holds the other streams' kernels)
-    ref_stages = stages_iso if stages_iso is not None else stages
-    dom = max(STAGES, key=lambda k: ref_stages[k]["ms_per_call"])
-    kern = {"calibrate": ("k_calibrate_prof" if fused else "k_calibrate") + " (+k_frame_sums)",
-            "estimate_shifts": "k_finalize, k_correlate (profile sums come from k_calibrate_prof)",
-            "resample": "k_resample<1> + k_ypass4 (x pass, y pass)" if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else "k_resample<0>",
-            "coadd": "k_coadd"}[dom]
-    traffic = None
-    tr_path = os.path.join(ROOT, "profiles", "traffic.csv")       # DRAM bytes per launch from the ncu --set full captures of config 2
-    if cfg == 2 and os.path.exists(tr_path):
-        for line in open(tr_path).read().splitlines()[1:]:
-            parts = line.split(",")
-            if parts and parts[0] == dom:
-                traffic = int(parts[1])
-    roof = {"bound": "hbm", "kernel": kern, "stage": dom, "achieved": ref_stages[dom]["GBps"], "peak": peak,
-            "peak_source": peak_src, "unit": "GB/s", "frac": ref_stages[dom]["frac"], "traffic": traffic,
-            "algorithmic_bytes_per_launch": sb[dom], "launch_ms": ref_stages[dom]["ms_per_call"],
-            "timing": ("CUDA events around the stage inside the C call, one stream (`stages_isolated`), same run"
-                       if stages_iso is not None else "CUDA events around the stage inside the C call, timed region"),
-            "frac_with_streams_overlapping": stages[dom]["frac"]}
-    sci_bytes = sum(sb[k] for k in STAGES)
-    sci_ms = sum(stages[k]["ms_per_call"] for k in STAGES)
-    e2e_roof = {"science_path_GBps": round(sci_bytes / (sci_ms * 1e-3) / 1e9, 1),
-                "science_path_frac": round(sci_bytes / (sci_ms * 1e-3) / 1e9 / peak, 4),
-                "whole_step_GBps": round((sci_bytes + sb["build_masters"]) * G / (total_ms / args.steps * 1e-3) / 1e9, 1)}
+            out[k] = {"ms_per_call": round(ms, 5), "algorithmic_MB": round(sb[k] / 1e6, 3), "GBps": round(gbs, 1),
+                      "frac": round(gbs / peak, 4)}
+        return out
+
+    stages = table(st_ms)
+    stages_iso = table(iso_ms) if iso_ms is not None else None
+    all_bytes = sum(sb[k] for k in ALL_STAGES)
+    whole_gbs = all_bytes * G * world / (total_ms / steps * 1e-3) / 1e9
+    res = dict(cfg=cfg, g=g, n=n, nm=nm, G=G, mode=mode, words=words, masked=any(b is not None for b in bad),
+               value=value, total_ms=total_ms, steps=steps, frames_per_step=frames_per_step, stages=stages,
+               stages_iso=stages_iso, clocks=clocks, graph=graph is not None, nstreams=len(streams), wall=wall,
+               peak=peak, peak_src=peak_src, sb=sb, whole_gbs=whole_gbs, e2e=None, truth=truth)
 
     # end to end through the C ABI with HOST buffers (H2D of every input and D2H of the result inside the region)
-    e2e = None
-    if not args.no_e2e:
+    if want_host:
         hplans = [mred.ReducePlan(g, n, device=devs, host=True) for _ in range(G)]
         stg = [{k: torch.empty_like(v) for k, v in d.items() if k != "sci"} for d in devg]
-
         masters_host = [None] * G
 
         def step_host():
@@ -432,9 +417,8 @@ def run_ours(args):
                 with torch.cuda.stream(st) if st is not None else contextlib.nullcontext():
                     for k in ("bias", "dark", "flat"):
                         stg[gi][k].copy_(host[gi][k], non_blocking=True)
-                    MB, MD, MF = mred.build_masters(g, stg[gi]["bias"], stg[gi]["dark"], groups[gi].t_dark,
-                                                    stg[gi]["flat"], groups[gi].t_flat, mode=mred.MEDIAN,
-                                                    ws=mwss[gi % len(streams)], out=masters_host[gi])
+                    MB, MD, MF = mred.build_masters(g, stg[gi]["bias"], stg[gi]["dark"], t_dark, stg[gi]["flat"], t_flat,
+                                                    mode=mred.MEDIAN, ws=mwss[gi % len(streams)], out=masters_host[gi])
                     masters_host[gi] = (MB, MD, MF)
                     mred.reduce_host(hplans[gi], host[gi]["sci"], scale, MB, MD, MF, 0, lag, badmask=bad[gi], mode=mode)
             for st in streams:
@@ -445,20 +429,104 @@ def run_ours(args):
         for _ in range(2):
             step_host()
         barrier()
-        ks = max(3, min(args.steps, 10))
+        ks = max(3, min(steps, 10))
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         for _ in range(ks):
             step_host()
         b.record()
         barrier()
-        ems = a.elapsed_time(b)
-        ems = max_over_ranks(ems, devs)
+        ems = max_over_ranks(a.elapsed_time(b), devs)
+        # the host path must give what the device path gives (bit for bit: tests/test_gpu_parity.py
+        # test_reduce_host_matches_reduce); checked here on the data just timed, so that a broken carve cannot print a number
+        same = all(bool(torch.equal(hplans[gi].out, plans[gi].out.cpu())) for gi in range(G))
         raw = 2 * g.W * g.H
-        e2e = {"value": frames_per_step * ks / (ems * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": G * (n + 3 * nm) * raw,
-               "d2h_bytes_per_step": G * (4 * g.w * g.h + 2 * g.w * g.h + 16 * n), "steps": ks,
-               "api": "mred_build_masters + mred_reduce_host (pinned host uint16 in, host float32 co-add out)"}
+        res["e2e"] = {"value": frames_per_step * ks / (ems * 1e-3), "unit": UNIT,
+                      "h2d_bytes_per_step": G * (n + 3 * nm) * raw,
+                      "d2h_bytes_per_step": G * (4 * g.w * g.h + 2 * g.w * g.h + 16 * n), "steps": ks,
+                      "api": "mred_build_masters + mred_reduce_host (pinned host uint16 in, host float32 co-add out)",
+                      "matches_device_path": same}
+    # free this config's device memory before the next one is set up
+    del devg, plans, mws, mwss, flush, masters_out, bad, host
+    torch.cuda.empty_cache()
+    return res
+
+
+def load_traffic(cfg):
+    """DRAM bytes per stage call (dram__bytes_read.sum + dram__bytes_write.sum of the stage's kernels) from the ncu
+    --set full capture of this round's build on this config: profiles/r2_traffic.csv, written from profiles/r2_kernels.md."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    out = {}
+    if os.path.exists(path):
+        for line in open(path).read().splitlines()[1:]:
+            parts = line.split(",")
+            if len(parts) >= 3 and parts[0].strip() == str(cfg):
+                out[parts[1].strip()] = int(float(parts[2]))
+    return out
+
+
+def summary(res):
+    ref = res["stages_iso"] if res["stages_iso"] is not None else res["stages"]
+    return {"workload": workload_name(res["cfg"]), "value": round(res["value"], 1), "unit": UNIT,
+            "ms_per_step": round(res["total_ms"] / res["steps"], 5), "steps": res["steps"],
+            "frames_per_step": res["frames_per_step"],
+            "whole_step_GBps": round(res["whole_gbs"], 1), "whole_step_frac": round(res["whole_gbs"] / res["peak"], 4),
+            "stage_frac_one_stream": {k: v["frac"] for k, v in ref.items()},
+            "stage_ms_one_stream": {k: v["ms_per_call"] for k, v in ref.items()},
+            "clocks": res["clocks"]}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2008_11486_b200 import binding as mred
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    devs = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=devs)
+    mred.lib()
+    cfg = args.config
+    res = bench_config(cfg, args, args.steps, max(args.warmup, 3), mred, torch, dist, devs, rank, world, local)
+    g, n, nm, G, mode = res["g"], res["n"], res["nm"], res["G"], res["mode"]
+    stages, stages_iso, sb, peak = res["stages"], res["stages_iso"], res["sb"], res["peak"]
+
+    # dominant stage over EVERY timed stage (build_masters included); its duration is taken without overlap from other
+    # groups when the step ran on several streams (an event interval on one stream then also holds the other streams' kernels)
+    ref_stages = stages_iso if stages_iso is not None else stages
+    dom = max(ALL_STAGES, key=lambda k: ref_stages[k]["ms_per_call"])
+    traffic = load_traffic(cfg)
+    roof = {"bound": "hbm", "kernel": stage_kernels(mred, g, n, mode)[dom], "stage": dom,
+            "achieved": ref_stages[dom]["GBps"], "peak": peak, "peak_source": res["peak_src"], "unit": "GB/s",
+            "frac": ref_stages[dom]["frac"], "traffic": traffic.get(dom),
+            "traffic_source": "profiles/r2_traffic.csv (ncu --set full of this build, config %d)" % cfg if dom in traffic else None,
+            "algorithmic_bytes_per_launch": sb[dom], "launch_ms": ref_stages[dom]["ms_per_call"],
+            "timing": ("CUDA events around the stage inside the C call, one stream (`stages_isolated`), same run"
+                       if stages_iso is not None else "CUDA events around the stage inside the C call, timed region"),
+            "frac_with_streams_overlapping": stages[dom]["frac"],
+            "all_stage_fracs": {k: ref_stages[k]["frac"] for k in ALL_STAGES}}
+    sci_bytes = sum(sb[k] for k in STAGES)
+    sci_ms = sum(ref_stages[k]["ms_per_call"] for k in STAGES)
+    path_roof = {"science_path_GBps_one_stream": round(sci_bytes / (sci_ms * 1e-3) / 1e9, 1),
+                 "science_path_frac_one_stream": round(sci_bytes / (sci_ms * 1e-3) / 1e9 / peak, 4),
+                 "whole_step_GBps": round(res["whole_gbs"], 1), "whole_step_frac": round(res["whole_gbs"] / peak, 4)}
+
+    # the other single-GPU configs, shorter runs of the same step, so that the driver's line carries them too
+    extra = {}
+    if rank == 0 and world == 1 and not args.no_extra:
+        for c in (2, 5):
+            if c == cfg:
+                continue
+            try:
+                r2 = bench_config(c, args, max(3, min(args.steps, 5)), 3, mred, torch, dist, devs, rank, world, local)
+                extra["config %d" % c] = summary(r2)
+            except Exception as exc:                     # an extra must never cost the headline
+                extra["config %d" % c] = {"error": repr(exc)[:200]}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -466,7 +534,7 @@ def run_ours(args):
         grp = synth.make_group(cfg, 0, **plan)
         s, nf, per, reps = 0.0, 0, {}, 0
         while s < 10.0 and reps < 50:                      # ~10-30 s of single-thread CPU work
-            s1, n1, p1 = time_oracle_group(grp, lag)
+            s1, n1, p1 = time_oracle_group(grp, MAX_LAG[cfg])
             s += s1
             nf += n1
             reps += 1
@@ -476,18 +544,21 @@ def run_ours(args):
                    reps, plan["n_sci"], plan["n_master"], plan["n_master"], plan["n_master"], cfg, s),
                "stage_seconds": {k: round(v, 3) for k, v in per.items()}, "host_cores_available": os.cpu_count()}
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": res["total_ms"] / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(cfg), "frames_per_step_per_gpu": G * n,
                            "includes": "build_masters + calibrate + estimate_shifts + resample + coadd per group",
                            "coadd": ["median", "mean", "sigclip 3.0 x3"][mode], "l2": "512 MB flush before every step",
-                           "parallelism": "groups sharded over ranks, no collective", "streams": len(streams), "launch": "cuda graph replay" if graph is not None else "plain launches",
+                           "parallelism": "groups sharded over ranks, no collective", "streams": res["nstreams"],
+                           "launch": "cuda graph replay" if res["graph"] else "plain launches",
                            "stage_timing": "CUDA events inside the C call; with a graph: instrumented plain-launch passes of the same step right after the timed region"},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * G * (KERNELS_PER_BUILD_MASTERS + (KERNELS_PER_REDUCE_FUSED + (1 if masked else 0)) + (1 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 0)),
-                "roofline": roof, "stages": stages, "stages_isolated": stages_iso, "path_roofline": e2e_roof, "cpu_baseline": cpu,
-                "wall_s_timed_region": round(wall, 4), "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU "
-                "stages on a TITAN X (Pascal) = ~870 frames/s (other hardware, other data; context only)"}
+                "clocks": res["clocks"], "e2e": res["e2e"],
+                "gpu_launches": args.steps * G * kernels_per_group(mred, g, n, res["masked"]),
+                "roofline": roof, "stages": stages, "stages_isolated": stages_iso, "path_roofline": path_roof,
+                "extra": extra, "cpu_baseline": cpu, "wall_s_timed_region": round(res["wall"], 4),
+                "paper_context": "PAPER.md Table 6: 540 frames in 0.621 s of GPU stages on a TITAN X (Pascal) = ~870 "
+                                 "frames/s (other hardware, other data; context only)"}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

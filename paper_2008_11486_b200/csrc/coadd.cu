@@ -237,11 +237,11 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
         static PerDeviceOnce once;
         int dev;
         if (once.pending(dev)) {
-            MRED_CUDA_TRY(cudaFuncSetAttribute(k_coadd_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, MRED_MAX_STACK * cs::TP * 4));
+            MRED_CUDA_TRY(cudaFuncSetAttribute(k_coadd_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, MRED_MAX_STACK * cs::TPS * 4));
             MRED_CUDA_TRY(cudaFuncSetAttribute(k_coadd_stream, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
             once.mark(dev);
         }
-        k_coadd_stream<<<dim3((unsigned)((np + cs::TP - 1) / cs::TP)), cs::TP, (size_t)n * cs::TP * 4, st>>>(
+        k_coadd_stream<<<dim3((unsigned)((np + cs::TP - 1) / cs::TP)), cs::TP, (size_t)n * cs::TPS * 4, st>>>(
             stack, n, w, h, fpd, use_fp, local, o.mode == MRED_SIGCLIP ? 1 : 0, ks, mi, out, count, rejmask);
         MRED_LAUNCH_CHECK();
         return MRED_OK;

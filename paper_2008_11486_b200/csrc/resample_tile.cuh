@@ -90,7 +90,7 @@ struct Seg {
     int r;                // 0..3: the strip's outputs sit r positions to the right of the box alignment
     int ylo, yhi;         // output rows of the segment that carry data (inclusive; ylo > yhi: none)
     int a0, nch;          // first source row of chunk 0 (may be negative), number of chunks
-    int kA;               // first interval (source row index) evaluated
+    int kA, kB;           // first and last interval (source row index) evaluated
     int pL, pR;           // warp position of image column 0 / w-1 when the box reaches beyond that edge, else -1
     Axis ax, ay;
 };
@@ -122,13 +122,13 @@ __device__ __forceinline__ Seg make_seg(long long item, int ya, int yb, int w, i
     g.ylo = max(ya, g.ay.lo);
     g.yhi = min(yb - 1, g.ay.hi);
     if (!x_any) { g.ylo = yb; g.yhi = yb - 1; }
-    g.a0 = 0; g.nch = 0; g.kA = 0;
+    g.a0 = 0; g.nch = 0; g.kA = 0; g.kB = -1;
     g.pL = (g.xsrc0 < 0 && -g.xsrc0 <= BOXW - 1) ? -g.xsrc0 : -1;
     const int pr = (w - 1) - g.xsrc0;
     g.pR = (pr >= 0 && pr < BOXW - 1) ? pr : -1;
     if (g.ylo > g.yhi) return g;
     const int kA = g.ylo + g.ay.m, kB = g.yhi + g.ay.m;       // intervals [kA, kB], inside [0, h-2] (identity axis: [0, h-1])
-    g.kA = kA;
+    g.kA = kA; g.kB = kB;
     if (g.ay.ident) {                                         // pure row translation: rows [kA, kB] are copied
         g.a0 = grid_floor(kA, h);
         g.nch = (kB - g.a0) / CH + 1;
@@ -151,17 +151,22 @@ struct YK {
     int my, ylo, yhi;    // interval k -> output row k - my, stored when in [ylo, yhi]
     float* po;           // output plane + the thread's column
     int w;
-    float fill;
-    bool in_fp;          // the column lies in the x footprint
 };
 
-__device__ __forceinline__ void emit(const YK& c, int k, float a0, float a1, float a2, float a3)
+// One output value = the 4 y taps.  FULL: the caller has established that every interval of the sweep is stored, and
+// walks `ptr` down the rows itself (two integer instructions per value instead of the guard, the multiplication by the
+// pitch and the 64-bit address of the general form: the store address arithmetic was 17 % of all instructions issued).
+template <bool FULL>
+__device__ __forceinline__ void emit(const YK& c, float*& ptr, int k, float a0, float a1, float a2, float a3)
 {
-    const int y = k - c.my;
-    if (y < c.ylo || y > c.yhi) return;          // block-uniform
-    float v = fmaf(c.w3, a3, fmaf(c.w2, a2, fmaf(c.w1, a1, c.w0 * a0)));
-    v = c.in_fp ? v : c.fill;
-    c.po[(size_t)((unsigned)y * (unsigned)c.w)] = v;
+    if (FULL) {
+        *ptr = fmaf(c.w3, a3, fmaf(c.w2, a2, fmaf(c.w1, a1, c.w0 * a0)));
+        ptr -= c.w;
+    } else {
+        const int y = k - c.my;
+        if (y < c.ylo || y > c.yhi) return;          // block-uniform
+        c.po[(size_t)((unsigned)y * (unsigned)c.w)] = fmaf(c.w3, a3, fmaf(c.w2, a2, fmaf(c.w1, a1, c.w0 * a0)));
+    }
 }
 
 // Anti-causal sweep of one chunk (rows a .. a+15 of the ring column Tc, stride TW) with the 4 y taps.
@@ -171,12 +176,15 @@ __device__ __forceinline__ void emit(const YK& c, int k, float a0, float a1, flo
 //            virtual c'[h] = 2 c'[h-1] - c'[h-2]; evaluates up to interval h-2.
 //   LOW:     rows below LOWROWS: elimination coefficients from the table, rows < -1 do not exist, row -1 is the virtual
 //            c'[-1] = 2 c'[0] - c'[1].
-template <bool LOW, bool FINAL>
+template <bool LOW, bool FINAL, bool FULL>
 __device__ __forceinline__ void sweep(const float* Tc, int a, float cstart, const YK& yk, float& s1, float& s2, float& s3)
 {
     constexpr int ITOP = FINAL ? CH - 2 : CH - 1;
+    constexpr int IEMIT = FINAL ? CH - 3 : CH - 4;          // first (highest) row of the sweep that completes an interval
     float c0 = FINAL ? Tc[(CH - 1) * TW] : cstart, c1 = 0.f, c2 = 0.f, c3 = 0.f;
     float n1 = c0, n2 = 0.f, n3 = 0.f;
+    float* ptr = yk.po;
+    if (FULL) ptr += (size_t)((unsigned)(a + IEMIT + 1 - yk.my) * (unsigned)yk.w);     // row of the highest interval
 #pragma unroll
     for (int i = ITOP; i >= 0; --i) {
         const int row = a + i;
@@ -192,13 +200,23 @@ __device__ __forceinline__ void sweep(const float* Tc, int a, float cstart, cons
         if (i == CH - 1) n1 = c0;
         if (i == CH - 2) n2 = c0;
         if (i == CH - 3) n3 = c0;
-        if (i <= (FINAL ? CH - 3 : CH - 4)) emit(yk, row + 1, c0, c1, c2, c3);
+        if (i <= IEMIT) emit<FULL>(yk, ptr, row + 1, c0, c1, c2, c3);
     }
     if (LOW && a == 0) s1 = fmaf(2.0f, c0, -c1);           // c'[-1] when row 0 opens the chunk
-    emit(yk, a, s1, c0, c1, c2);
-    emit(yk, a - 1, s2, s1, c0, c1);
-    emit(yk, a - 2, s3, s2, s1, c0);
+    emit<FULL>(yk, ptr, a, s1, c0, c1, c2);
+    emit<FULL>(yk, ptr, a - 1, s2, s1, c0, c1);
+    emit<FULL>(yk, ptr, a - 2, s3, s2, s1, c0);
     s1 = n1; s2 = n2; s3 = n3;
+}
+
+// block-uniform dispatch: FULL when every interval the sweep evaluates (a-2 .. top) is stored
+template <bool LOW, bool FINAL>
+__device__ __forceinline__ void sweep_any(const float* Tc, int a, float cstart, const YK& yk, int kA, int kB, float& s1,
+                                          float& s2, float& s3)
+{
+    const int ktop = a + (FINAL ? CH - 2 : CH - 3);
+    if (a - 2 >= kA && ktop <= kB) sweep<LOW, FINAL, true>(Tc, a, cstart, yk, s1, s2, s3);
+    else sweep<LOW, FINAL, false>(Tc, a, cstart, yk, s1, s2, s3);
 }
 
 // Causal pass of one chunk in place (T -> g) and the look-ahead sum A = c'[a] seen from the chunk before.
@@ -241,6 +259,15 @@ __device__ __forceinline__ void shift_left(float (&f)[V])
     for (int j = 0; j + R < V; ++j) f[j] = f[j + R];
 #pragma unroll
     for (int j = 0; j < R; ++j) f[V - R + j] = nx[j];
+}
+
+__device__ __forceinline__ void store_rows(float* t0, bool keep, const float (&f)[2][V])
+{
+    if (!keep) return;
+    *reinterpret_cast<float4*>(t0) = make_float4(f[0][0], f[0][1], f[0][2], f[0][3]);
+    *reinterpret_cast<float4*>(t0 + 4) = make_float4(f[0][4], f[0][5], f[0][6], f[0][7]);
+    *reinterpret_cast<float4*>(t0 + TW) = make_float4(f[1][0], f[1][1], f[1][2], f[1][3]);
+    *reinterpret_cast<float4*>(t0 + TW + 4) = make_float4(f[1][4], f[1][5], f[1][6], f[1][7]);
 }
 
 // The reflected halo of one staged row: positions left of image column 0 (at warp position pL) and right of column
@@ -313,19 +340,38 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
     const long long u0 = (long long)blockIdx.x * per_cta, u1 = min(units, u0 + per_cta);
     if (u0 >= u1) return;
 
-    Walker wk;                                   // the producer's view (thread 0): NSTAGE chunks ahead of the consumers
+    // The last warp has no column in the y pass (208 columns = 6.5 warps): its first lane is the producer (NSTAGE chunks
+    // ahead of the consumers), and the warp is the only one that polls an mbarrier; everybody else learns that a chunk
+    // has landed from the block barrier that follows (256 polling threads cost issue slots the other CTAs could use).
+    constexpr int PW = NTHR / 32 - 1;
+    Walker wk;
     wk.u = u0; wk.u1 = u1; wk.j = 0; wk.nch = 0; wk.x = 0; wk.a0 = 0; wk.z = 0;
-    if (tid == 0) {
-        for (int i = 0; i < NSTAGE; ++i) {
-            Box b;
-            if (!wk.next(b, w, h, ns, hs, dshift)) break;
-            mbar_arrive_expect_tx(&full[i], STAGE_FLOATS * 4);
-            tma_load_3d(stage + i * STAGE_FLOATS, &tmap, b.x, b.y, b.z, &full[i]);
-        }
+    int total = 0;                               // chunks of this CTA
+    for (long long uu = u0; uu < u1;) {
+        const long long item = uu / h;
+        const int ya = (int)(uu - item * h);
+        const int len = (int)min((long long)(h - ya), u1 - uu);
+        total += make_seg(item, ya, ya + len, w, h, ns, hs, dshift).nch;
+        uu += len;
     }
+    if (warp == PW) {
+        if (lane == 0) {
+            for (int i = 0; i < NSTAGE; ++i) {
+                Box b;
+                if (!wk.next(b, w, h, ns, hs, dshift)) break;
+                mbar_arrive_expect_tx(&full[i], STAGE_FLOATS * 4);
+                tma_load_3d(stage + i * STAGE_FLOATS, &tmap, b.x, b.y, b.z, &full[i]);
+            }
+        }
+        __syncwarp();
+        if (total > 0) mbar_wait(&full[0], 0);
+    }
+    __syncthreads();
+    int done = 0;                                // chunks consumed
 
     const size_t np = (size_t)w * h;
-    unsigned gc = 0;                             // chunks consumed so far: stage = gc % NSTAGE, phase = (gc / NSTAGE) & 1
+    int st = 0;                                  // stage of the next chunk and the parity of its mbarrier phase
+    unsigned ph = 0;
     long long u = u0;
     while (u < u1) {
         const long long item = u / h;
@@ -357,22 +403,24 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
         const bool edge = sg.pL >= 0 || sg.pR >= 0;
         // y-pass constants of this thread's column
         const int col = sg.Xs + tid;
-        const bool ycol = tid < TW && col < sg.Xe;
+        bool ycol = tid < TW && col < sg.Xe;
         YK yk;
         yk.na = -U_INF;
         const float scy = sg.ay.ident ? 1.f : 6.0f * U_INF;
         yk.w0 = scy * sg.ay.w[0]; yk.w1 = scy * sg.ay.w[1]; yk.w2 = scy * sg.ay.w[2]; yk.w3 = scy * sg.ay.w[3];
         yk.my = sg.ay.m; yk.ylo = sg.ylo; yk.yhi = sg.yhi;
         yk.po = outk + (ycol ? col : sg.Xs);
-        yk.w = w; yk.fill = fill;
-        yk.in_fp = col >= sg.ax.lo && col <= sg.ax.hi;
+        yk.w = w;
+        if (ycol && !(col >= sg.ax.lo && col <= sg.ax.hi)) {
+            // a column outside the x footprint: fill, for every row of the segment that carries data; nothing else to do
+            for (int y = sg.ylo; y <= sg.yhi; ++y) yk.po[(size_t)((unsigned)y * (unsigned)w)] = fill;
+            ycol = false;
+        }
         float gprev = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
 
-        for (int j = 0; j < sg.nch; ++j, ++gc) {
-            const int st = gc % NSTAGE;
+        for (int j = 0; j < sg.nch; ++j) {
             const int a = sg.a0 + CH * j;                               // first source row of the chunk
-            float* T = tring + (j % NT) * T_FLOATS;
-            mbar_wait(&full[st], (gc / NSTAGE) & 1u);
+            float* T = tring + (j % NT) * T_FLOATS;      // (the chunk's box has landed: see the end of the iteration before)
             // ---------------- x pass: warp = rows 2 warp, 2 warp + 1
             {
                 const int i0 = 2 * warp;
@@ -397,27 +445,30 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
                         f[1][4] = q1.x; f[1][5] = q1.y; f[1][6] = q1.z; f[1][7] = q1.w;
                     }
                     rs::x_pass<2>(nax, nax8, wx, f);
-                    switch (sg.r) {                                     // warp-uniform: outputs move r positions left
-                        case 1: shift_left<1>(f[0]); shift_left<1>(f[1]); break;
-                        case 2: shift_left<2>(f[0]); shift_left<2>(f[1]); break;
-                        case 3: shift_left<3>(f[0]); shift_left<3>(f[1]); break;
-                        default: break;
-                    }
-                    if (lane >= HL && lane < 32 - HL) {
-                        float* t0 = T + i0 * TW + V * (lane - HL);
-                        *reinterpret_cast<float4*>(t0) = make_float4(f[0][0], f[0][1], f[0][2], f[0][3]);
-                        *reinterpret_cast<float4*>(t0 + 4) = make_float4(f[0][4], f[0][5], f[0][6], f[0][7]);
-                        *reinterpret_cast<float4*>(t0 + TW) = make_float4(f[1][0], f[1][1], f[1][2], f[1][3]);
-                        *reinterpret_cast<float4*>(t0 + TW + 4) = make_float4(f[1][4], f[1][5], f[1][6], f[1][7]);
+                    float* t0 = T + i0 * TW + V * (lane - HL);
+                    const bool keep = lane >= HL && lane < 32 - HL;
+                    switch (sg.r) {          // warp-uniform: the outputs move r positions left (each case stores by itself:
+                                             // a common store after the switch would cost 16 register moves per pair of rows)
+                        case 0: store_rows(t0, keep, f); break;
+                        case 1: shift_left<1>(f[0]); shift_left<1>(f[1]); store_rows(t0, keep, f); break;
+                        case 2: shift_left<2>(f[0]); shift_left<2>(f[1]); store_rows(t0, keep, f); break;
+                        default: shift_left<3>(f[0]); shift_left<3>(f[1]); store_rows(t0, keep, f); break;
                     }
                 }
             }
             __syncthreads();                    // the chunk's x-shifted rows are complete; its stage is free again
-            if (tid == 0) {
-                Box b;
-                if (wk.next(b, w, h, ns, hs, dshift)) {
-                    mbar_arrive_expect_tx(&full[st], STAGE_FLOATS * 4);
-                    tma_load_3d(stage + st * STAGE_FLOATS, &tmap, b.x, b.y, b.z, &full[st]);
+            if (warp == PW) {
+                if (lane == 0) {
+                    Box b;
+                    if (wk.next(b, w, h, ns, hs, dshift)) {
+                        mbar_arrive_expect_tx(&full[st], STAGE_FLOATS * 4);
+                        tma_load_3d(stage + st * STAGE_FLOATS, &tmap, b.x, b.y, b.z, &full[st]);
+                    }
+                }
+                __syncwarp();
+                if (done + 1 < total) {             // wait for the next chunk while the other warps run the y pass
+                    const int nst = st + 1 == NSTAGE ? 0 : st + 1;
+                    mbar_wait(&full[nst], nst == 0 ? ph ^ 1u : ph);
                 }
             }
             // ---------------- y pass: thread = column
@@ -428,7 +479,7 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
 #pragma unroll 4
                     for (int i = 0; i < CH; ++i) {
                         const int y = a + i - yk.my;
-                        if (y >= yk.ylo && y <= yk.yhi) yk.po[(size_t)((unsigned)y * (unsigned)w)] = yk.in_fp ? Tc[i * TW] : fill;
+                        if (y >= yk.ylo && y <= yk.yhi) yk.po[(size_t)((unsigned)y * (unsigned)w)] = Tc[i * TW];
                     }
                 } else {
                     const bool is_final = a + CH == h;
@@ -436,13 +487,16 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
                     const float A = low ? causal<true>(Tc, a, is_final, yk.na, gprev) : causal<false>(Tc, a, is_final, yk.na, gprev);
                     if (j >= 1 && a - 1 >= sg.kA - 1) {                  // the chunk before holds rows that are evaluated
                         const float* Tp = tring + ((j - 1) % NT) * T_FLOATS + tid;
-                        if (a - CH <= CH) sweep<true, false>(Tp, a - CH, A, yk, s1, s2, s3);
-                        else sweep<false, false>(Tp, a - CH, A, yk, s1, s2, s3);
+                        if (a - CH <= CH) sweep_any<true, false>(Tp, a - CH, A, yk, sg.kA, sg.kB, s1, s2, s3);
+                        else sweep_any<false, false>(Tp, a - CH, A, yk, sg.kA, sg.kB, s1, s2, s3);
                     }
-                    if (is_final && a + CH - 1 >= sg.kA - 1) sweep<false, true>(Tc, a, 0.f, yk, s1, s2, s3);
+                    if (is_final && a + CH - 1 >= sg.kA - 1) sweep_any<false, true>(Tc, a, 0.f, yk, sg.kA, sg.kB, s1, s2, s3);
                 }
             }
-            if (NT == 2) __syncthreads();       // the ring slot of chunk j-1 is written again by the x pass of chunk j+1
+            __syncthreads();                    // the next chunk has landed (seen by the last warp); with NT == 2 also: the
+                                                // ring slot of chunk j-1 is written again by the x pass of chunk j+1
+            ++done;
+            if (++st == NSTAGE) { st = 0; ph ^= 1u; }
         }
     }
 }

@@ -34,6 +34,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity)
 // instead of hanging the device.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
+    if (mbar_try_wait(bar, parity)) return;      // the usual case: the box landed while the chunk before was worked on
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity))
         if (++spins > (1u << 24)) {

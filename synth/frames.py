@@ -46,7 +46,7 @@ GEOM_PAPER = Geom(1074, 1024, 0, 50, 52, 2, 1020, 1020)       # 10
 GEOM_LARGE = Geom(4128, 4096, 0, 32, 32, 0, 4096, 4096)       # BASELINE.json config 5
 GEOM_SMALL = Geom(210, 136, 0, 18, 18, 0, 192, 136)           # test-size stand-in, same structure
 
-# combine modes (values match include/mred.h and oracle/mred_oracle.h by convention only)
+# combine modes (values match include/mred.h and oracle/mred_oracle.c by convention only)
 MEDIAN, MEAN, SIGCLIP = 0, 1, 2
 
 CONFIGS = {
@@ -122,8 +122,19 @@ def _draw_shifts(rng, n, S):
     return sh
 
 
+def _map(fn, items, workers):
+    """Frames are drawn from independent generators (one SeedSequence path each), so they can be made in any order
+    and on several threads (numpy releases the GIL while it draws) with the same result."""
+    items = list(items)
+    if workers and workers > 1 and len(items) > 1:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=min(workers, len(items))) as ex:
+            return list(ex.map(fn, items))
+    return [fn(i) for i in items]
+
+
 def make_group(config: int, group: int = 0, *, geom: Geom | None = None, n_sci=None, n_master=None,
-               stars=None, S=None, seed=None, masters: bool = True, science: bool = True):
+               stars=None, S=None, seed=None, masters: bool = True, science: bool = True, workers: int = 0):
     """One (telescope, band) group of BASELINE.json config `config`.
 
     Returns a namespace with uint16 stacks bias/dark/flat/sci of shape [n][H][W], exposure
@@ -141,11 +152,11 @@ def make_group(config: int, group: int = 0, *, geom: Geom | None = None, n_sci=N
                           bias=None, dark=None, flat=None, sci=None, shifts=None, badmask=None, sky=None)
     nm = sp["n_master"]
     if masters:
-        out.bias = np.stack([_finish(_rng(seed, 1, k), g, np.zeros((g.H, g.W)), rn) for k in range(nm)])
-        out.dark = np.stack([_finish(_rng(seed, 2, k), g, np.full((g.H, g.W), DARK_RATE * T_DARK), rn)
-                             for k in range(nm)])
-        out.flat = np.stack([_finish(_rng(seed, 3, k), g, flat * FLAT_LEVEL + DARK_RATE * T_FLAT, rn)
-                             for k in range(nm)])
+        out.bias = np.stack(_map(lambda k: _finish(_rng(seed, 1, k), g, np.zeros((g.H, g.W)), rn), range(nm), workers))
+        out.dark = np.stack(_map(lambda k: _finish(_rng(seed, 2, k), g, np.full((g.H, g.W), DARK_RATE * T_DARK), rn),
+                                 range(nm), workers))
+        out.flat = np.stack(_map(lambda k: _finish(_rng(seed, 3, k), g, flat * FLAT_LEVEL + DARK_RATE * T_FLAT, rn),
+                                 range(nm), workers))
     if not science:
         return out
     n = sp["n_sci"]
@@ -167,8 +178,7 @@ def make_group(config: int, group: int = 0, *, geom: Geom | None = None, n_sci=N
         hot_amp = r0.uniform(2000.0, 20000.0, size=nh)
         out.badmask = np.zeros((g.h, g.w), dtype=np.uint8)
         out.badmask[:, hot_cols] = 1
-    frames = []
-    for k in range(n):
+    def one_frame(k):
         rk = _rng(seed, 5, k)
         model = skies[k] + _render_stars(g, sx + shifts[k, 0], sy + shifts[k, 1], peaks)
         el = flat * model + DARK_RATE * T_SCI
@@ -187,8 +197,9 @@ def make_group(config: int, group: int = 0, *, geom: Geom | None = None, n_sci=N
                     Y = cy[j] + (0 if horiz[j] else s)
                     if X < g.W and Y < g.H:
                         el[Y, X] += amp[j]
-        frames.append(_finish(rk, g, el, rn))
-    out.sci = np.stack(frames)
+        return _finish(rk, g, el, rn)
+
+    out.sci = np.stack(_map(one_frame, range(n), workers))
     out.shifts = shifts
     out.sky = skies
     return out
