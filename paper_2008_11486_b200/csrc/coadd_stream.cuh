@@ -269,9 +269,12 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
             r2 = group_sum(r2, L, gmask);
             cnt -= rc;
             if (cnt == 0) break;
+            const float dm = -r1 / (float)cnt;               // the survivors' deviations summed to -r1: their mean moves by dm
+            mean += dm;
             if (r2 > 0.25f * S) {
-                // what left carried a good part of S (a cosmic ray, a hot column): S - r2 would cancel, so the moments of
-                // the survivors are taken again, about the old mean, in a sweep of their own
+                // what left carried a good part of S (a cosmic ray, a hot column): S - r2 would cancel, so the second moment
+                // of the survivors is taken again, about the new mean, in a sweep of its own (q1 mops up what dm lost
+                // to rounding next to the outlier)
                 float q1 = 0.f, q2 = 0.f;
                 for (int k = sub; k < n; k += L) { const float t = (cq[k * TPS] - c) - mean; if (t == t) { q1 += t; q2 = fmaf(t, t, q2); } }
                 q1 = group_sum(q1, L, gmask);
@@ -279,18 +282,7 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
                 const float dq = q1 / (float)cnt;
                 mean += dq;
                 S = fmaxf(q2 - dq * q1, 0.f);
-                if (dq * dq * (float)cnt > 0.25f * S) {      // the mean itself moved by a good part of sigma: once more about it
-                    q1 = 0.f; q2 = 0.f;
-                    for (int k = sub; k < n; k += L) { const float t = (cq[k * TPS] - c) - mean; if (t == t) { q1 += t; q2 = fmaf(t, t, q2); } }
-                    q1 = group_sum(q1, L, gmask);
-                    q2 = group_sum(q2, L, gmask);
-                    const float d2 = q1 / (float)cnt;
-                    mean += d2;
-                    S = fmaxf(q2 - d2 * q1, 0.f);
-                }
             } else {
-                const float dm = -r1 / (float)cnt;           // the survivors' deviations summed to -r1
-                mean += dm;
                 S = fmaxf((S - r2) - dm * dm * (float)cnt, 0.f);
             }
         }

@@ -16,7 +16,8 @@ namespace mred {
 struct MastersWs {            // layout of the caller's workspace (all 16-byte aligned)
     unsigned long long* os;   // [nb + nd + nf] overscan sums (bias, dark, flat frames in that order)
     unsigned long long* img_f;// [nf] image-rectangle sums of the flats
-    unsigned int* ticket;     // [2] block counters of the two combine kernels (zeroed with the sums)
+    unsigned int* ticket;     // [3] block counters of the two combine kernels and of the sums kernel (zeroed with the sums)
+    float* lev;               // [nb + nd + nf] overscan levels as float32 (written by the last block of k_master_sums)
     double* part_bd;          // [nblocks][2] block sums of MB, MD
     double* part_f;           // [nblocks]    block sums of the un-normalised MF
     float* inv_gm;            // [nf] 1/<G_k>
@@ -40,6 +41,7 @@ static MastersWs carve(void* ws, const Geom& g, int nb, int nd, int nf)
     m.part_bd = reinterpret_cast<double*>(take(16 * nblocks));
     m.part_f = reinterpret_cast<double*>(take(8 * nblocks));
     m.inv_gm = reinterpret_cast<float*>(take(4 * (size_t)nf));
+    m.lev = reinterpret_cast<float*>(take(4 * (size_t)(nb + nd + nf)));
     m.inv_mf = reinterpret_cast<float*>(take(16));
     m.bytes = (size_t)(p - static_cast<char*>(ws));
     return m;
@@ -57,90 +59,68 @@ __global__ void __launch_bounds__(256) k_master_sums(const uint16_t* __restrict_
                                                      const uint16_t* __restrict__ dark, int nd,
                                                      const uint16_t* __restrict__ flat, int nf, Geom g, int nos, int nimg,
                                                      unsigned long long* __restrict__ os,
-                                                     unsigned long long* __restrict__ img_f, int pair_ok)
+                                                     unsigned long long* __restrict__ img_f, unsigned int* __restrict__ ticket,
+                                                     float* __restrict__ lev, int pair_ok)
 {
+    __shared__ unsigned long long s_w[8];
     const size_t fs = (size_t)g.W * g.H;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nall = nb + nd + nf;
     int b = blockIdx.x;
+    unsigned long long* dst;
+    unsigned long long s = 0;
     if (b < nos * nall) {
         const int k = b / nos, c = b - k * nos;
         const uint16_t* f = k < nb ? bias + (size_t)k * fs : (k < nb + nd ? dark + (size_t)(k - nb) * fs : flat + (size_t)(k - nb - nd) * fs);
         const int r = c * blockDim.x + threadIdx.x;
-        unsigned long long s = 0;
         if (r < g.H && g.os_x1 > g.os_x0) s = overscan_row_sum(f, g.W, g.os_x0, g.os_x1, r);
-        s = warp_sum(s);
-        __shared__ unsigned long long s_w[8];
-        if (lane == 0) s_w[warp] = s;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            unsigned long long t = 0;
-            for (int i = 0; i < 8; ++i) t += s_w[i];
-            if (t) atomicAdd(os + k, t);
-        }
-        return;
-    }
-    b -= nos * nall;                               // image sums: flats only
-    const int kf = b / nimg, c = b - kf * nimg;
-    const uint16_t* f = flat + (size_t)kf * fs;
-    const int r = g.y0 + c * 8 + warp;
-    __shared__ unsigned long long s_b[8];
-    const bool live = r < g.y0 + g.h;
-    const uint16_t* row = f + (size_t)(live ? r : g.y0) * g.W;
-    unsigned long long bsum = 0;
-    if (!live) {
-    } else if (pair_ok) {      // two pixels per 32-bit load, 16 independent loads in flight
-        const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
-        const int w2 = g.w >> 1;
-        int x = lane;
-        for (; x + 15 * 32 < w2; x += 16 * 32) {
-            unsigned int v[16];
-#pragma unroll
-            for (int u = 0; u < 16; ++u) v[u] = __ldg(row2 + x + 32 * u);
-            unsigned int t = 0;
-#pragma unroll
-            for (int u = 0; u < 16; ++u) t += (v[u] & 0xffffu) + (v[u] >> 16);     // 32 x 65535 < 2^32
-            bsum += t;
-        }
-        for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); bsum += (v & 0xffffu) + (v >> 16); }
+        dst = os + k;
     } else {
-        for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) bsum += __ldg(row + x);
+        b -= nos * nall;                               // image sums: flats only
+        const int kf = b / nimg, c = b - kf * nimg;
+        const uint16_t* f = flat + (size_t)kf * fs;
+        const int r = g.y0 + c * 8 + warp;
+        const bool live = r < g.y0 + g.h;
+        const uint16_t* row = f + (size_t)(live ? r : g.y0) * g.W;
+        if (!live) {
+        } else if (pair_ok) {      // two pixels per 32-bit load, 16 independent loads in flight
+            const unsigned int* row2 = reinterpret_cast<const unsigned int*>(row + g.x0);
+            const int w2 = g.w >> 1;
+            int x = lane;
+            for (; x + 15 * 32 < w2; x += 16 * 32) {
+                unsigned int v[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) v[u] = __ldg(row2 + x + 32 * u);
+                unsigned int t = 0;
+#pragma unroll
+                for (int u = 0; u < 16; ++u) t += (v[u] & 0xffffu) + (v[u] >> 16);     // 32 x 65535 < 2^32
+                s += t;
+            }
+            for (; x < w2; x += 32) { const unsigned int v = __ldg(row2 + x); s += (v & 0xffffu) + (v >> 16); }
+        } else {
+            for (int x = g.x0 + lane; x < g.x0 + g.w; x += 32) s += __ldg(row + x);
+        }
+        dst = img_f + kf;
     }
-    bsum = warp_sum(bsum);
-    if (lane == 0) s_b[warp] = bsum;
+    s = warp_sum(s);
+    if (lane == 0) s_w[warp] = s;
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (warp != 0) return;
+    // warp 0: the block's total, then the ticket; the LAST block to arrive turns every overscan sum into its float32 level
+    // (one float64 division per frame, done once here instead of by every block of the combine kernels)
+    int last = 0;
+    if (lane == 0) {
         unsigned long long t = 0;
-        for (int i = 0; i < 8; ++i) t += s_b[i];
-        if (t) atomicAdd(img_f + kf, t);
+        for (int i = 0; i < 8; ++i) t += s_w[i];
+        if (t) atomicAdd(dst, t);
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     }
-}
-
-// deterministic block sum of one double per thread (256 threads): shuffle tree, then warp 0 adds the
-// eight warp totals in index order.  Result valid in thread 0.
-__device__ __forceinline__ double block_sum_256f(float v, double* s8)
-{
-    v = warp_sum(v);          // 32 lanes x <= 2 pixels in float32: relative error 1e-6 of a block partial, far below
-                              // what <MB>, <MD>, <MF> need (they enter <G_k> ~ 2e4 ADU to 1e-7 relative)
-    if ((threadIdx.x & 31) == 0) s8[threadIdx.x >> 5] = (double)v;
-    __syncthreads();
-    double t = 0.0;
-    if (threadIdx.x == 0)
-        for (int i = 0; i < 8; ++i) t += s8[i];
-    __syncthreads();
-    return t;
-}
-
-__device__ __forceinline__ double block_sum_256(double v, double* s8)
-{
-    v = warp_sum(v);
-    if ((threadIdx.x & 31) == 0) s8[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double t = 0.0;
-    if (threadIdx.x == 0)
-        for (int i = 0; i < 8; ++i) t += s8[i];
-    __syncthreads();
-    return t;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (!last) return;
+    __threadfence();
+    const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
+    for (int k = lane; k < nall; k += 32) lev[k] = cnt > 0 ? (float)((double)__ldcg(os + k) / (double)cnt) : 0.f;
 }
 
 template <int NMAX, int MODE>
@@ -150,29 +130,28 @@ __device__ __forceinline__ float combine_all(float (&v)[NMAX], int n, float ksig
     return combine_mean_clip<NMAX>(v, n, MODE == MRED_SIGCLIP, ksigma, max_iter).value;
 }
 
-// PX pixels of frame k starting at element q of the frame (PX = 2: one aligned 32-bit load)
-template <int PX>
-__device__ __forceinline__ void load_px(const uint16_t* f, size_t q, int nv, float (&o)[PX])
+// PX pixels of one frame at p (PX = 2: one aligned 32-bit load).  uint16 -> float32 stays on the conversion unit (I2F.U16
+// picks its half of the register by itself, so the unpacking costs no ALU instruction): these kernels are bound by the ALU
+// pipe (FMNMX of the median network, 70 % busy at N = 20), and the PRMT + FADD form that avoids I2F measured 3 % slower.
+// base + k frames: one 32 x 32 -> 64-bit multiply-add (IMAD.WIDE.U32, FMA pipe) per load.  A frame is < 2^31 pixels
+// (geom_ok), so its size in bytes fits 32 bits; pointer increments would cost two ALU-pipe additions per load, and the
+// ALU pipe is what bounds these kernels.
+__device__ __forceinline__ const uint16_t* frame_ptr(const uint16_t* base, int k, unsigned int frame_bytes)
 {
-    if (PX == 2) {
-        const unsigned int v = __ldcs(reinterpret_cast<const unsigned int*>(f + q));
-        o[0] = (float)(v & 0xffffu); o[PX - 1] = (float)(v >> 16);
-    } else {
-#pragma unroll
-        for (int i = 0; i < PX; ++i) o[i] = i < nv ? (float)__ldcs(f + q + i) : 0.f;
-    }
+    return reinterpret_cast<const uint16_t*>(reinterpret_cast<const char*>(base) + (unsigned long long)(unsigned int)k * frame_bytes);
 }
 
-// true in exactly one block: the last one to arrive (its reads of the other blocks' partial sums are ordered
-// by the fence / atomic pair)
-__device__ __forceinline__ bool last_block(unsigned int* ticket)
+template <int PX>
+__device__ __forceinline__ void load_px(const uint16_t* p, int nv, float (&o)[PX])
 {
-    __shared__ int s_last;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
-    __syncthreads();
-    return s_last != 0;
+    if (PX == 2) {
+        const unsigned int v = __ldcs(reinterpret_cast<const unsigned int*>(p));
+        o[0] = (float)(v & 0xffffu);
+        o[PX - 1] = (float)(v >> 16);
+    } else {
+#pragma unroll
+        for (int i = 0; i < PX; ++i) o[i] = i < nv ? (float)__ldcs(p + i) : 0.f;
+    }
 }
 
 // ---- bias + dark; the last block turns the block sums into 1/<G_k> of every flat ----------------
@@ -185,13 +164,12 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
                                                     float* __restrict__ MB, float* __restrict__ MD)
 {
     __shared__ float s_lb[MRED_MAX_STACK + 1], s_ld[MRED_MAX_STACK + 1];
-    __shared__ double s8[8];
-    __shared__ double s_mean[2];
     const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
-    for (int k = threadIdx.x; k < nb; k += blockDim.x) s_lb[k] = cnt > 0 ? (float)((double)m.os[k] / (double)cnt) : 0.f;
-    for (int k = threadIdx.x; k < nd; k += blockDim.x) s_ld[k] = cnt > 0 ? (float)((double)m.os[nb + k] / (double)cnt) : 0.f;
+    for (int k = threadIdx.x; k < nb; k += blockDim.x) s_lb[k] = m.lev[k];
+    for (int k = threadIdx.x; k < nd; k += blockDim.x) s_ld[k] = m.lev[nb + k];
     __syncthreads();
     const size_t fs = (size_t)g.W * g.H;
+    const unsigned int fsb = (unsigned int)(fs * 2);
     const int wg = (g.w + PX - 1) / PX;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
@@ -206,15 +184,15 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
         float v[PX][NMAX], dk[PX][NMAX];
         const uint16_t* pb = bias + q;
         const uint16_t* pd = dark + q;
-        // every load of both stacks is issued before the first median starts
+        // every load of both stacks is issued before the first median starts (address = base + k * frame: one
+        // multiply-add per load)
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX], od[PX];
 #pragma unroll
             for (int i = 0; i < PX; ++i) { o[i] = 0.f; od[i] = 0.f; }
-            if (FULL || k < nb) load_px<PX>(pb, 0, nv, o);
-            if (FULL || k < nd) load_px<PX>(pd, 0, nv, od);
-            pb += fs; pd += fs;
+            if (FULL || k < nb) load_px<PX>(frame_ptr(pb, k, fsb), nv, o);
+            if (FULL || k < nd) load_px<PX>(frame_ptr(pd, k, fsb), nv, od);
 #pragma unroll
             for (int i = 0; i < PX; ++i) { v[i][k] = (FULL || k < nb) ? o[i] - s_lb[k] : ABSENT; dk[i][k] = od[i]; }
         }
@@ -240,35 +218,38 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
     float tb = 0.f, td = 0.f;
 #pragma unroll
     for (int i = 0; i < PX; ++i) { tb += mb[i]; td += md[i]; }
-    // block partials of both planes and the "last block" ticket with two barriers in all
+    // block partials of both planes; after the one barrier only warp 0 stays: it writes the partials and takes the ticket,
+    // and in the LAST block to arrive it adds up all partials (fixed order) and turns them into 1/<G_k>.  (With the whole
+    // block waiting for the fence + ticket round trip, "barrier" was the top stall reason of this kernel.)
     __shared__ float2 s_w2[8];
-    __shared__ int s_lastb;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     tb = warp_sum(tb);          // <= 64 values of one plane in float32: 1e-6 relative on a partial
     td = warp_sum(td);
-    if ((threadIdx.x & 31) == 0) s_w2[threadIdx.x >> 5] = make_float2(tb, td);
+    if (lane == 0) s_w2[warp] = make_float2(tb, td);
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (warp != 0) return;
+    int last = 0;
+    if (lane == 0) {
         double sb = 0.0, sd = 0.0;
         for (int i = 0; i < 8; ++i) { sb += (double)s_w2[i].x; sd += (double)s_w2[i].y; }
         m.part_bd[2 * (size_t)blockIdx.x] = sb;
         m.part_bd[2 * (size_t)blockIdx.x + 1] = sd;
         __threadfence();
-        s_lastb = (atomicAdd(m.ticket, 1u) == gridDim.x - 1);
+        last = atomicAdd(m.ticket, 1u) == gridDim.x - 1;
     }
-    __syncthreads();
-    if (!s_lastb) return;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (!last) return;
     __threadfence();
     // <G_k> = <F_k> - L_k - <MB> - r <MD>: fixed-order sums of the block partials
     double a = 0.0, b = 0.0;
-    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) { a += __ldcg(m.part_bd + 2 * (size_t)i); b += __ldcg(m.part_bd + 2 * (size_t)i + 1); }
-    const double sa = block_sum_256(a, s8);
-    const double sbb = block_sum_256(b, s8);
+    for (int i = lane; i < (int)gridDim.x; i += 32) { a += __ldcg(m.part_bd + 2 * (size_t)i); b += __ldcg(m.part_bd + 2 * (size_t)i + 1); }
+    a = warp_sum(a);
+    b = warp_sum(b);
     const double np = (double)g.w * (double)g.h;
-    if (threadIdx.x == 0) { s_mean[0] = sa / np; s_mean[1] = sbb / np; }
-    __syncthreads();
-    for (int k = threadIdx.x; k < nf; k += blockDim.x) {
-        const double L = cnt > 0 ? (double)m.os[nb + nd + k] / (double)cnt : 0.0;
-        const double gm = (double)m.img_f[k] / np - L - s_mean[0] - r * s_mean[1];
+    const double mean_b = a / np, mean_d = b / np;
+    for (int k = lane; k < nf; k += 32) {
+        const double L = cnt > 0 ? (double)__ldcg(m.os + nb + nd + k) / (double)cnt : 0.0;
+        const double gm = (double)__ldcg(m.img_f + k) / np - L - mean_b - r * mean_d;
         m.inv_gm[k] = (float)(1.0 / gm);
     }
 }
@@ -281,14 +262,13 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
                                                    float* __restrict__ MF)
 {
     __shared__ float s_lf[MRED_MAX_STACK + 1], s_ig[MRED_MAX_STACK + 1];
-    __shared__ double s8[8];
-    const long long cnt = (long long)(g.os_x1 - g.os_x0) * g.H;
     for (int k = threadIdx.x; k < nf; k += blockDim.x) {
-        s_lf[k] = cnt > 0 ? (float)((double)m.os[nb + nd + k] / (double)cnt) : 0.f;
+        s_lf[k] = m.lev[nb + nd + k];
         s_ig[k] = m.inv_gm[k];
     }
     __syncthreads();
     const size_t fs = (size_t)g.W * g.H;
+    const unsigned int fsb = (unsigned int)(fs * 2);
     const int wg = (g.w + PX - 1) / PX;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
@@ -308,8 +288,7 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX];
-            if (FULL || k < nf) load_px<PX>(pf, 0, nv, o);
-            pf += fs;
+            if (FULL || k < nf) load_px<PX>(frame_ptr(pf, k, fsb), nv, o);
 #pragma unroll
             for (int i = 0; i < PX; ++i) v[i][k] = (FULL || k < nf) ? ((o[i] - s_lf[k]) - off[i]) * s_ig[k] : ABSENT;
         }
@@ -325,24 +304,26 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
 #pragma unroll
     for (int i = 0; i < PX; ++i) t += mf[i];
     __shared__ float s_w1[8];
-    __shared__ int s_lastb;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     t = warp_sum(t);
-    if ((threadIdx.x & 31) == 0) s_w1[threadIdx.x >> 5] = t;
+    if (lane == 0) s_w1[warp] = t;
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (warp != 0) return;                 // only warp 0 waits for the ticket (see k_masters_bd)
+    int last = 0;
+    if (lane == 0) {
         double sblk = 0.0;
         for (int i = 0; i < 8; ++i) sblk += (double)s_w1[i];
         m.part_f[blockIdx.x] = sblk;
         __threadfence();
-        s_lastb = (atomicAdd(m.ticket + 1, 1u) == gridDim.x - 1);
+        last = atomicAdd(m.ticket + 1, 1u) == gridDim.x - 1;
     }
-    __syncthreads();
-    if (!s_lastb) return;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (!last) return;
     __threadfence();
     double a = 0.0;
-    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) a += __ldcg(m.part_f + i);
-    const double sall = block_sum_256(a, s8);
-    if (threadIdx.x == 0) m.inv_mf[0] = (float)((double)g.w * (double)g.h / sall);
+    for (int i = lane; i < (int)gridDim.x; i += 32) a += __ldcg(m.part_f + i);
+    a = warp_sum(a);
+    if (lane == 0) m.inv_mf[0] = (float)((double)g.w * (double)g.h / a);
 }
 
 __global__ void __launch_bounds__(256) k_mf_scale(float* __restrict__ MF, size_t np, const float* __restrict__ inv_mf, int vec)
@@ -414,7 +395,7 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     // pairs of pixels by one 32-bit load need even W, x0 and w (frame bases are 16-byte aligned, frames W*H*2 B)
     const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0 && g.w % 2 == 0 && ((size_t)g.W * g.H) % 2 == 0) ? 1 : 0;
     const int nos = (g.H + 255) / 256, nimg = (g.h + 7) / 8;
-    k_master_sums<<<dim3((unsigned)(nos * (nb + nd + nf) + nimg * nf)), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, nos, nimg, m.os, m.img_f, pair_ok);
+    k_master_sums<<<dim3((unsigned)(nos * (nb + nd + nf) + nimg * nf)), 256, 0, st>>>(bias, nb, dark, nd, flat, nf, g, nos, nimg, m.os, m.img_f, m.ticket + 2, m.lev, pair_ok);
     MRED_LAUNCH_CHECK();
     const size_t np = (size_t)g.w * g.h;
     const int nbd = nb > nd ? nb : nd;
