@@ -13,12 +13,12 @@
 //           (max |v - mu| > k sigma).  If not -- most pixels -- the result is the mean of everything, exactly what O6 says.
 //   pass B  the "dirty" pixels of the block (15-20 % at N = 60, 3 sigma) are compacted, and L lanes share each of them
 //           (L = 128 / dirty count, a power of two: frames k = sub, sub + L, ..), so the block's threads stay busy and the
-//           serial chains are L times shorter.  A clip pass is a sweep of 4 instructions per value (load, two subtractions,
-//           compare); only a REJECTED value does more: it is marked NaN in shared memory and taken out of the running
-//           count, sum and sum of squares, from which the next mean and sigma follow (sum_kept (t - dm)^2 = S - sum_rej t^2
-//           - cnt dm^2, all terms of order N sigma^2; when one outlier carries a quarter of S the moments are taken again
-//           in a sweep of their own, so nothing cancels).  The passes start from pass A's statistics.  The rejection mask
-//           is read off the NaN marks.  Without compaction every warp would run three masked passes for its few dirty lanes.
+//           serial chains are L times shorter.  A clip pass is one branch-free sweep (cs::clip_dirty); what it rejects is
+//           marked NaN in shared memory and its count, sum and sum of squares give the next mean and sigma (sum_kept
+//           (t - dm)^2 = S - sum_rej t^2 - cnt dm^2, all terms of order N sigma^2; when one outlier carries a quarter of S
+//           the second moment is taken again in a sweep of its own, so nothing cancels).  The passes start from pass A's
+//           statistics.  The rejection mask is read off the NaN marks.  Without compaction every warp would run three
+//           masked passes for its few dirty lanes.
 // Frames whose footprint does not cover the whole tile take the general branch of pass A (per-pixel test, absent = NaN).
 // HBM traffic: N * 4 B read + 4 + 2 (+ 4 ceil(N/32)) B written per pixel; requires w * h % 4 == 0 (16-byte aligned tiles).
 #pragma once
@@ -37,16 +37,106 @@ __device__ __forceinline__ float median3(float a, float b, float c)
     return fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));
 }
 
-// sum over the L lanes (L a power of two, lanes aligned to L) that share a pixel; every lane gets the total
-__device__ __forceinline__ float group_sum(float v, int L, unsigned gmask)
+struct ClipArgs {
+    float* vals; const short* list; const float *c0, *mean, *S; const short* m;
+    int n, nd; float ksigma; int max_iter; size_t p0, np;
+    float* out; uint16_t* count; uint32_t* rejmask;
+};
+
+template <int L>
+__device__ __forceinline__ float gsum(float v, unsigned gmask)
 {
+#pragma unroll
     for (int o = L >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(gmask, v, o);
     return v;
 }
-__device__ __forceinline__ int group_sum(int v, int L, unsigned gmask)
+template <int L>
+__device__ __forceinline__ int gsum(int v, unsigned gmask)
 {
+#pragma unroll
     for (int o = L >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(gmask, v, o);
     return v;
+}
+
+// The clip loop of O6 on the dirty columns.  L lanes share a column: lane `sub` owns frames sub, sub + L, ...  A pass is
+// ONE branch-free sweep (per value: load, two subtractions, compare, select, two accumulates, a predicated count and a
+// predicated store of the NaN mark): with 16 columns per warp some lane rejects at almost every step, so a branch around
+// the "rare" rejection would be taken all the time.  The survivors' moments are accumulated about the column's provisional
+// centre c (pass A: the median of three frames, within a sigma of the survivors' mean whatever the outliers are), NOT about
+// the mean that is being clipped against, which still holds the outliers: so mean' = m1 / cnt and S' = m2 - mean' m1 do
+// not cancel even when a 60000-ADU hit has just left, and no second sweep is needed.  Only a centre that was an outlier
+// itself (|mean'| > 4 sigma) is moved and the moments taken again.  NaN = not used.
+template <int L>
+__device__ __forceinline__ void clip_dirty(const ClipArgs& a, int tid)
+{
+    const int lane = tid & 31, sub = tid & (L - 1);
+    const unsigned gmask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (lane & ~(L - 1)));
+    const int n = a.n;
+    constexpr int STEP = L * TPS;                            // this lane's next frame is L rows on
+    for (int gi = tid / L; gi < a.nd; gi += TP / L) {
+        const int q = a.list[gi];
+        const size_t pq = a.p0 + q;
+        float* cq = a.vals + q + sub * TPS;
+        const int nk = (n - sub + L - 1) / L;                // frames of this lane
+        int cnt = a.m[q];
+        float c = a.c0[q], mean = a.mean[q], S = a.S[q];
+        bool recentre = cnt < 0;
+        cnt = recentre ? -cnt : cnt;
+        for (int it = 0; it < a.max_iter; ++it) {
+            if (recentre) {                                  // group-uniform, rare: centre on the survivors' mean
+                c += mean;
+                float t1 = 0.f, t2 = 0.f;
+#pragma unroll 4
+                for (int i = 0; i < nk; ++i) { float d = cq[i * STEP] - c; d = (d == d) ? d : 0.f; t1 += d; t2 = fmaf(d, d, t2); }
+                t1 = gsum<L>(t1, gmask);
+                t2 = gsum<L>(t2, gmask);
+                mean = t1 / (float)cnt;
+                S = fmaxf(t2 - mean * t1, 0.f);
+            }
+            const float thr = fmaf(a.ksigma, sqrtf(S / (float)cnt), 1e-10f * fabsf(c));
+            float m1 = 0.f, m2 = 0.f;                        // survivors: sum and sum of squares of v - c
+            int ncnt = 0;
+#pragma unroll 4
+            for (int i = 0; i < nk; ++i) {
+                const float u = cq[i * STEP] - c;
+                const bool keep = fabsf(u - mean) <= thr;    // false for NaN (absent / rejected before)
+                const float uk = keep ? u : 0.f;
+                m1 += uk;
+                m2 = fmaf(uk, uk, m2);
+                ncnt += keep ? 1 : 0;
+                if (!keep) cq[i * STEP] = CUDART_NAN_F;      // a predicated store
+            }
+            ncnt = gsum<L>(ncnt, gmask);
+            if (ncnt == cnt) break;                          // group-uniform: nothing rejected
+            cnt = ncnt;
+            if (cnt == 0) break;
+            m1 = gsum<L>(m1, gmask);
+            m2 = gsum<L>(m2, gmask);
+            mean = m1 / (float)cnt;
+            S = fmaxf(m2 - mean * m1, 0.f);
+            recentre = mean * mean * (float)cnt > 16.0f * S;
+        }
+        if (sub == 0) {
+            a.out[pq] = cnt > 0 ? c + mean : 0.f;
+            if (a.count) a.count[pq] = (uint16_t)cnt;
+        }
+        if (a.rejmask) {
+            // mask words from the NaN marks; L divides 32, so word wd holds this lane's frames i in [wd 32/L, (wd+1) 32/L)
+            constexpr int PER = 32 / L;
+            const int words = (n + 31) >> 5;
+            for (int wd = 0; wd < words; ++wd) {
+                uint32_t bits = 0u;
+#pragma unroll
+                for (int j = 0; j < PER; ++j) {
+                    const int i = wd * PER + j;
+                    if (i < nk) { const float v = cq[i * STEP]; if (!(v == v)) bits |= 1u << (sub + j * L); }
+                }
+#pragma unroll
+                for (int o = L >> 1; o > 0; o >>= 1) bits |= __shfl_xor_sync(gmask, bits, o);
+                if (sub == 0) a.rejmask[(size_t)wd * a.np + pq] = bits;
+            }
+        }
+    }
 }
 
 }  // namespace cs
@@ -226,80 +316,18 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
     __syncthreads();
     const int nd = s_nd;
     if (nd == 0) return;
-    // ---- pass B: the clip loop (same float operations as combine_mean_clip, combine.cuh) on the dirty columns, L lanes per
-    // column (L = the largest power of two that lets the block take all of them at once): each lane owns frames
-    // sub, sub + L, ..; the three sums of a pass are reduced over the group by shuffles.  NaN = not used.
+    // ---- pass B on the compacted dirty columns, L lanes per column (the largest power of two that lets the block take all
+    // of them at once)
     int L = 1;
     while (L < 32 && 2 * L * nd <= TP && 2 * L <= n) L <<= 1;
-    const int sub = tid & (L - 1);
-    const unsigned gmask = (L == 32) ? 0xffffffffu : (((1u << L) - 1u) << (lane & ~(L - 1)));
-    for (int gi = tid / L; gi < nd; gi += TP / L) {
-        const int q = s_list[gi];
-        const size_t pq = p0 + q;
-        float* cq = vals + q;
-        int cnt = s_m[q];
-        float c = s_c0[q], mean = s_mean[q], S = s_S[q];
-        if (cnt < 0) {                                       // take the moments again about the mean
-            cnt = -cnt;
-            float sum = 0.f;
-            for (int k = sub; k < n; k += L) { const float v = cq[k * TPS]; if (v == v) sum += v; }
-            c = group_sum(sum, L, gmask) / (float)cnt;
-            float t1 = 0.f, t2 = 0.f;
-            for (int k = sub; k < n; k += L) { const float d = cq[k * TPS] - c; if (d == d) { t1 += d; t2 = fmaf(d, d, t2); } }
-            t1 = group_sum(t1, L, gmask);
-            t2 = group_sum(t2, L, gmask);
-            mean = t1 / (float)cnt;
-            S = fmaxf(t2 - mean * t1, 0.f);
-        }
-        // mean, S: mean and centred sum of squares of the cnt survivors, both about c (sum of (v - c) - mean over them = 0)
-        for (int it = 0; it < max_iter; ++it) {
-            const float thr = fmaf(ksigma, sqrtf(S / (float)cnt), 1e-10f * fabsf(c));
-            float r1 = 0.f, r2 = 0.f;                        // sum and sum of squares of what this pass rejects
-            int rc = 0;
-            for (int k = sub; k < n; k += L) {
-                const float t = (cq[k * TPS] - c) - mean;
-                if (fabsf(t) > thr) {                        // false for NaN (absent / rejected before)
-                    cq[k * TPS] = CUDART_NAN_F;
-                    ++rc; r1 += t; r2 = fmaf(t, t, r2);
-                }
-            }
-            rc = group_sum(rc, L, gmask);
-            if (rc == 0) break;                              // group-uniform: nothing rejected
-            r1 = group_sum(r1, L, gmask);
-            r2 = group_sum(r2, L, gmask);
-            cnt -= rc;
-            if (cnt == 0) break;
-            const float dm = -r1 / (float)cnt;               // the survivors' deviations summed to -r1: their mean moves by dm
-            mean += dm;
-            if (r2 > 0.25f * S) {
-                // what left carried a good part of S (a cosmic ray, a hot column): S - r2 would cancel, so the second moment
-                // of the survivors is taken again, about the new mean, in a sweep of its own (q1 mops up what dm lost
-                // to rounding next to the outlier)
-                float q1 = 0.f, q2 = 0.f;
-                for (int k = sub; k < n; k += L) { const float t = (cq[k * TPS] - c) - mean; if (t == t) { q1 += t; q2 = fmaf(t, t, q2); } }
-                q1 = group_sum(q1, L, gmask);
-                q2 = group_sum(q2, L, gmask);
-                const float dq = q1 / (float)cnt;
-                mean += dq;
-                S = fmaxf(q2 - dq * q1, 0.f);
-            } else {
-                S = fmaxf((S - r2) - dm * dm * (float)cnt, 0.f);
-            }
-        }
-        if (sub == 0) {
-            out[pq] = cnt > 0 ? c + mean : 0.f;
-            if (count) count[pq] = (uint16_t)cnt;
-        }
-        if (rejmask) {
-            __syncwarp(gmask);                               // the NaN marks of the other lanes of the group
-            for (int wd = 0; wd < words; ++wd) {
-                uint32_t bits = 0u;
-                const int k0 = 32 * wd, k1 = min(n, k0 + 32);
-                for (int k = k0 + sub; k < k1; k += L) { const float v = cq[k * TPS]; if (!(v == v)) bits |= 1u << (k - k0); }
-                for (int o = L >> 1; o > 0; o >>= 1) bits |= __shfl_xor_sync(gmask, bits, o);
-                if (sub == 0) rejmask[(size_t)wd * np + pq] = bits;
-            }
-        }
+    const ClipArgs ca{vals, s_list, s_c0, s_mean, s_S, s_m, n, nd, ksigma, max_iter, p0, np, out, count, rejmask};
+    switch (L) {
+        case 1: clip_dirty<1>(ca, tid); break;
+        case 2: clip_dirty<2>(ca, tid); break;
+        case 4: clip_dirty<4>(ca, tid); break;
+        case 8: clip_dirty<8>(ca, tid); break;
+        case 16: clip_dirty<16>(ca, tid); break;
+        default: clip_dirty<32>(ca, tid); break;
     }
 }
 
