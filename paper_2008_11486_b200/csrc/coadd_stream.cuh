@@ -155,13 +155,14 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
     __shared__ short s_list[TP];
     __shared__ float s_c0[TP], s_mean[TP], s_S[TP];         // pass A's statistics of the dirty pixels, for pass B
     __shared__ short s_m[TP];                               // values in the column; negative: statistics unusable (recentre)
-    __shared__ int s_nall, s_nnone, s_nd;
+    __shared__ unsigned char s_nfl[MRED_MAX_STACK + 1];     // the frames that do not cover the whole tile (any order)
+    __shared__ int s_nall, s_nnone, s_nd, s_nnf;
     const int tid = threadIdx.x, lane = tid & 31;
     const size_t np = (size_t)w * h;
     const size_t p0 = (size_t)blockIdx.x * TP;
     const int tp = (int)min((size_t)TP, np - p0);           // pixels of this tile (a multiple of 4)
     if (tid == 0) {
-        s_nall = 0; s_nnone = 0; s_nd = 0;
+        s_nall = 0; s_nnone = 0; s_nd = 0; s_nnf = 0;
         tma::mbar_init(&s_bar, 1);
         tma::fence_mbar_init();
     }
@@ -185,6 +186,7 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
             }
             s_cls[k] = (unsigned char)cls;
             if (cls == 1) atomicAdd(&s_nall, 1);
+            else s_nfl[atomicAdd(&s_nnf, 1)] = (unsigned char)k;
             if (cls == 0) atomicAdd(&s_nnone, 1);
         }
     }
@@ -215,14 +217,12 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
         if (!fast) {
             // frames that do not cover this pixel become NaN in the staged column: absent, like a rejected value
             const int y = (int)((unsigned)p / (unsigned)w), x = (int)((unsigned)p - (unsigned)y * (unsigned)w);
-            for (int k = 0; k < n; ++k) {
-                const int cls = s_cls[k];
-                if (cls == 1) continue;                      // block-uniform
-                bool ok = false;
-                if (cls == 2) {
-                    const int4 f = fp_dev ? fp_dev[k] : hfp.fp[k];
-                    ok = x >= f.x && x <= f.y && y >= f.z && y <= f.w;
-                }
+            const int nnf = s_nnf;
+            for (int i = 0; i < nnf; ++i) {                  // only the frames that miss part of the tile
+                const int k = s_nfl[i];
+                const int4 f = fp_dev ? fp_dev[k] : hfp.fp[k];
+                const bool ok = (unsigned)(x - f.x) <= (unsigned)(f.y - f.x) && (unsigned)(y - f.z) <= (unsigned)(f.w - f.z) &&
+                                f.x <= f.y && f.z <= f.w;
                 if (!ok) col[k * TPS] = CUDART_NAN_F;
             }
         }
