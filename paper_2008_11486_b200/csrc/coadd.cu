@@ -231,7 +231,7 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
     const int4* fpd = reinterpret_cast<const int4*>(fp_dev);
     const float ks = o.ksigma;
     const int mi = o.max_iter;
-    if (o.mode != MRED_MEDIAN && np % 4 == 0) {
+    if (o.mode != MRED_MEDIAN && np % 4 == 0 && np >= (size_t)cs::TPS) {
         // mean / sigma-clipped mean: streaming pass + compacted clip pass on bulk-copy-staged tiles (coadd_stream.cuh);
         // planes whose size is not a multiple of 4 pixels (tiles not 16-byte aligned) keep the register kernels below
         static PerDeviceOnce once;
@@ -241,8 +241,13 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
             MRED_CUDA_TRY(cudaFuncSetAttribute(k_coadd_stream, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
             once.mark(dev);
         }
+        CUtensorMap tm;
+        const cuuint64_t dims[2] = {(cuuint64_t)np, (cuuint64_t)n};
+        const cuuint64_t strides[1] = {(cuuint64_t)np * 4};
+        const cuuint32_t box[2] = {(cuuint32_t)cs::TPS, (cuuint32_t)n};
+        if (!tma::encode_f32_map(&tm, stack, 2, dims, strides, box)) { set_cuda_error(cudaErrorInvalidValue); return MRED_ECUDA; }
         k_coadd_stream<<<dim3((unsigned)((np + cs::TP - 1) / cs::TP)), cs::TP, (size_t)n * cs::TPS * 4, st>>>(
-            stack, n, w, h, fpd, use_fp, local, o.mode == MRED_SIGCLIP ? 1 : 0, ks, mi, out, count, rejmask);
+            tm, n, w, h, fpd, use_fp, local, o.mode == MRED_SIGCLIP ? 1 : 0, ks, mi, out, count, rejmask);
         MRED_LAUNCH_CHECK();
         return MRED_OK;
     }

@@ -4,9 +4,9 @@
 // Why: a thread that keeps its pixel's whole N-frame column in registers and runs up to three clip passes over it issues
 // ~27 instructions per value; at N = 60 that is issue-bound at about a third of the HBM rate, with 200+ registers per
 // thread and 8 warps per SM.  But a clip pass only matters for the pixels where it rejects something.  So:
-//   stage   a block owns 128 consecutive pixels.  Warp 0 issues one 512-byte bulk copy (cp.async.bulk, completion on an
-//           mbarrier) per frame: the [N][128] tile lands in shared memory with no register staging, and with 7 blocks per
-//           SM at N = 60 some 200 KB per SM are in flight.
+//   stage   a block owns 128 consecutive pixels.  One cp.async.bulk.tensor box (132 pixels x N frames through a 2-D tensor
+//           map over the [N][w*h] stack, completion on an mbarrier) brings the whole tile into shared memory with no
+//           register staging; with 6 blocks per SM at N = 60 some 190 KB per SM are in flight.
 //   pass A  thread = pixel, ONE sweep down its column in shared memory with O(1) state: moments about a provisional
 //           centre (the median of the first three frames), minimum and maximum.  6 instructions per value, ~30 registers.
 //           From these: the mean, the population sigma, and whether the first clip pass would reject anything at all
@@ -141,8 +141,8 @@ __device__ __forceinline__ void clip_dirty(const ClipArgs& a, int tid)
 
 }  // namespace cs
 
-// grid (ceil(np / 128)), block 128, dynamic shared memory n * 528 bytes
-__global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict__ stack, int n, int w, int h,
+// grid (ceil(np / 128)), block 128, dynamic shared memory n * 528 bytes; tmap: dims {w*h, n}, box {132, n}
+__global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__ CUtensorMap tmap, int n, int w, int h,
                                                          const int4* __restrict__ fp_dev, int use_fp,
                                                          const __grid_constant__ HostFootprints hfp, int clip, float ksigma,
                                                          int max_iter, float* __restrict__ out, uint16_t* __restrict__ count,
@@ -191,12 +191,13 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const float* __restrict
         }
     }
     __syncthreads();
-    // stage the tile: one bulk copy per frame that touches it
-    if (tid < 32) {
-        if (lane == 0) tma::mbar_arrive_expect_tx(&s_bar, (uint32_t)(n - s_nnone) * (uint32_t)tp * 4u);
-        __syncwarp();
-        for (int k = lane; k < n; k += 32)
-            if (s_cls[k]) tma::bulk_load(vals + k * TPS, stack + (size_t)k * np + p0, (uint32_t)tp * 4u, &s_bar);
+    // stage the tile: ONE tensor copy, a box of TPS pixels x n frames out of the [n][w*h] stack.  (One 512-byte bulk copy
+    // per frame, 60 per tile, held the whole kernel at 3.5 TB/s: the copy engine takes a copy every ~40 cycles per SM
+    // whatever its size.)  The box is 4 pixels wider than the tile, so the rows land with the 132-float pitch that keeps
+    // pass B free of bank conflicts; pixels beyond the plane arrive as zeros and are never looked at.
+    if (tid == 0) {
+        tma::mbar_arrive_expect_tx(&s_bar, (uint32_t)n * (uint32_t)TPS * 4u);
+        tma::tma_load_2d(vals, &tmap, (int)p0, 0, &s_bar);
     }
     const bool live = tid < tp;
     const size_t p = p0 + tid;

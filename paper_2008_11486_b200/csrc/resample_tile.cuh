@@ -24,7 +24,6 @@
 // plane re-reads 17-32 rows of warm-up.
 #pragma once
 #include "tma.cuh"
-#include <cudaTypedefs.h>   // PFN_cuTensorMapEncodeTiled_v12000
 
 namespace mred {
 namespace rt {
@@ -503,21 +502,6 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
 
 namespace rt {
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point query: libmred.so links only the CUDA runtime
-inline PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder()
-{
-    static std::atomic<void*> cached{nullptr};
-    void* p = cached.load(std::memory_order_acquire);
-    if (!p) {
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
-            q != cudaDriverEntryPointSuccess)
-            return nullptr;
-        cached.store(p, std::memory_order_release);
-    }
-    return reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
-}
-
 inline bool tile_route(int w, int h) { return (w % 4 == 0) && w >= MIN_W && h >= MIN_H; }
 
 constexpr int TILE_NT = 2;
@@ -525,19 +509,11 @@ constexpr int TILE_NT = 2;
 inline int launch_resample_tile(const float* in, int n, int w, int h, const HostShifts& hs, const double* dshift_dev,
                                 float fill, float* out, int4* fpd, cudaStream_t st)
 {
-    auto encode = tensor_map_encoder();
-    if (!encode) { set_cuda_error(cudaErrorSymbolNotFound); return MRED_ECUDA; }
     CUtensorMap tm;
     const cuuint64_t dims[3] = {(cuuint64_t)w, (cuuint64_t)h, (cuuint64_t)n};
     const cuuint64_t strides[2] = {(cuuint64_t)w * 4, (cuuint64_t)w * (cuuint64_t)h * 4};
     const cuuint32_t box[3] = {BOXW, CH, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(in), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
-        set_cuda_error(cudaErrorInvalidValue);
-        return MRED_ECUDA;
-    }
+    if (!tma::encode_f32_map(&tm, in, 3, dims, strides, box)) { set_cuda_error(cudaErrorInvalidValue); return MRED_ECUDA; }
     constexpr size_t smem = smem_bytes<TILE_NT>();
     static PerDeviceOnce once;
     static std::atomic<int> occ_cache[64];

@@ -2,6 +2,9 @@
 // cp.async.bulk.tensor).  SASS: SYNCS.*, UBLKCP, UTMALDG.
 #pragma once
 #include <cuda.h>           // CUtensorMap and its enums (types only: the encoder is fetched through the runtime)
+#include <cudaTypedefs.h>   // PFN_cuTensorMapEncodeTiled_v12000
+#include <cuda_runtime.h>
+#include <atomic>
 #include <cstdio>
 #include <stdint.h>
 
@@ -50,6 +53,14 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
         : "memory");
 }
 
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int x, int y, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(smem_u32(bar))
+        : "memory");
+}
+
 // 1-D bulk copy global -> shared: dst, src 16-byte aligned, bytes a multiple of 16; completion counted on `bar`
 __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
 {
@@ -58,6 +69,33 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
                  : "memory");
 }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point query: libmred.so links only the CUDA runtime
+inline PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder()
+{
+    static std::atomic<void*> cached{nullptr};
+    void* p = cached.load(std::memory_order_acquire);
+    if (!p) {
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        cached.store(p, std::memory_order_release);
+    }
+    return reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+}
+
+// float32 tensor map of rank 2 or 3 (dims, box: innermost first; strides in bytes for dims 1..rank-1); false on failure
+inline bool encode_f32_map(CUtensorMap* tm, const float* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                           const cuuint32_t* box)
+{
+    auto encode = tensor_map_encoder();
+    if (!encode) return false;
+    const cuuint32_t estr[3] = {1, 1, 1};
+    return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<float*>(base), dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 }  // namespace tma
 }  // namespace mred
