@@ -143,32 +143,63 @@ __device__ __forceinline__ Seg make_seg(long long item, int ya, int yb, int w, i
     return g;
 }
 
-// y-pass constants of one segment, per thread (= per column)
+// ---- y pass: a thread owns CY adjacent columns.  CY = 2 (64-bit shared-memory and global accesses, half the load / store /
+// address instructions per pixel) was MEASURED SLOWER than CY = 1: config 3 192 us against 153 us, config 5 3.81 ms against
+// 3.10 ms -- the y phase then runs in 3.25 warps per CTA instead of 6.5 and its dependent chains are no longer hidden.
+constexpr int CY = 1;
+struct F2 { float x, y; };
+template <int C> struct ValT { using type = float; };
+template <> struct ValT<2> { using type = F2; };
+using VT = ValT<CY>::type;
+
+__device__ __forceinline__ float vfma(float s, float a, float b) { return fmaf(s, a, b); }
+__device__ __forceinline__ F2 vfma(float s, F2 a, F2 b) { return F2{fmaf(s, a.x, b.x), fmaf(s, a.y, b.y)}; }
+__device__ __forceinline__ float vmul(float s, float a) { return s * a; }
+__device__ __forceinline__ F2 vmul(float s, F2 a) { return F2{s * a.x, s * a.y}; }
+__device__ __forceinline__ float vext(float c0, float c1) { return fmaf(2.0f, c0, -c1); }            // 2 c0 - c1
+__device__ __forceinline__ F2 vext(F2 c0, F2 c1) { return F2{fmaf(2.0f, c0.x, -c1.x), fmaf(2.0f, c0.y, -c1.y)}; }
+__device__ __forceinline__ void vzero(float& v) { v = 0.f; }
+__device__ __forceinline__ void vzero(F2& v) { v.x = 0.f; v.y = 0.f; }
+__device__ __forceinline__ void vld(const float* p, float& v) { v = *p; }
+__device__ __forceinline__ void vld(const float* p, F2& v) { const float2 t = *reinterpret_cast<const float2*>(p); v.x = t.x; v.y = t.y; }
+__device__ __forceinline__ void vst(float* p, float v) { *p = v; }
+__device__ __forceinline__ void vst(float* p, F2 v) { *reinterpret_cast<float2*>(p) = make_float2(v.x, v.y); }
+
+// y-pass constants of one segment, per thread
 struct YK {
     float na;            // -a
     float w0, w1, w2, w3;// the four weights times 6a
     int my, ylo, yhi;    // interval k -> output row k - my, stored when in [ylo, yhi]
-    float* po;           // output plane + the thread's column
+    float* po;           // output plane + the thread's first column
     int w;
+    bool in0, in1;       // CY = 2: which of the two columns lie in the x footprint (at least one does)
 };
+
+__device__ __forceinline__ void put(const YK& c, float* p, float v) { *p = v; }
+__device__ __forceinline__ void put(const YK& c, float* p, F2 v)
+{
+    if (c.in0 && c.in1) *reinterpret_cast<float2*>(p) = make_float2(v.x, v.y);      // all but the two columns at a footprint edge
+    else if (c.in0) p[0] = v.x;
+    else p[1] = v.y;
+}
 
 // One output value = the 4 y taps.  FULL: the caller has established that every interval of the sweep is stored, and
 // walks `ptr` down the rows itself (two integer instructions per value instead of the guard, the multiplication by the
 // pitch and the 64-bit address of the general form: the store address arithmetic was 17 % of all instructions issued).
 template <bool FULL>
-__device__ __forceinline__ void emit(const YK& c, float*& ptr, int k, float a0, float a1, float a2, float a3)
+__device__ __forceinline__ void emit(const YK& c, float*& ptr, int k, VT a0, VT a1, VT a2, VT a3)
 {
     if (FULL) {
-        *ptr = fmaf(c.w3, a3, fmaf(c.w2, a2, fmaf(c.w1, a1, c.w0 * a0)));
+        put(c, ptr, vfma(c.w3, a3, vfma(c.w2, a2, vfma(c.w1, a1, vmul(c.w0, a0)))));
         ptr -= c.w;
     } else {
         const int y = k - c.my;
         if (y < c.ylo || y > c.yhi) return;          // block-uniform
-        c.po[(size_t)((unsigned)y * (unsigned)c.w)] = fmaf(c.w3, a3, fmaf(c.w2, a2, fmaf(c.w1, a1, c.w0 * a0)));
+        put(c, c.po + (size_t)((unsigned)y * (unsigned)c.w), vfma(c.w3, a3, vfma(c.w2, a2, vfma(c.w1, a1, vmul(c.w0, a0)))));
     }
 }
 
-// Anti-causal sweep of one chunk (rows a .. a+15 of the ring column Tc, stride TW) with the 4 y taps.
+// Anti-causal sweep of one chunk (rows a .. a+15 of the ring columns at Tc, row stride TW) with the 4 y taps.
 //   REGULAR: cstart = c'[a+16] from the look-ahead of the chunk that follows; evaluates intervals a-2 .. a+13, the three
 //            that reach into the chunk before with the values s1..s3 = c'[a-1], c'[a-2], c'[a-3] that chunk left.
 //   FINAL:   the chunk ends with the last row of the plane: c'[h-1] is stored in the ring (exact end condition), the
@@ -176,32 +207,37 @@ __device__ __forceinline__ void emit(const YK& c, float*& ptr, int k, float a0, 
 //   LOW:     rows below LOWROWS: elimination coefficients from the table, rows < -1 do not exist, row -1 is the virtual
 //            c'[-1] = 2 c'[0] - c'[1].
 template <bool LOW, bool FINAL, bool FULL>
-__device__ __forceinline__ void sweep(const float* Tc, int a, float cstart, const YK& yk, float& s1, float& s2, float& s3)
+__device__ __forceinline__ void sweep(const float* Tc, int a, VT cstart, const YK& yk, VT& s1, VT& s2, VT& s3)
 {
     constexpr int ITOP = FINAL ? CH - 2 : CH - 1;
     constexpr int IEMIT = FINAL ? CH - 3 : CH - 4;          // first (highest) row of the sweep that completes an interval
-    float c0 = FINAL ? Tc[(CH - 1) * TW] : cstart, c1 = 0.f, c2 = 0.f, c3 = 0.f;
-    float n1 = c0, n2 = 0.f, n3 = 0.f;
+    VT c0 = cstart, c1, c2, c3, n1, n2, n3;
+    if (FINAL) vld(Tc + (CH - 1) * TW, c0);
+    vzero(c1); vzero(c2); vzero(c3); vzero(n2); vzero(n3);
+    n1 = c0;
     float* ptr = yk.po;
     if (FULL) ptr += (size_t)((unsigned)(a + IEMIT + 1 - yk.my) * (unsigned)yk.w);     // row of the highest interval
 #pragma unroll
     for (int i = ITOP; i >= 0; --i) {
         const int row = a + i;
-        float cn;
+        VT cn;
         if (!LOW || row >= 0) {
-            const float g = Tc[i * TW];
-            cn = LOW ? fmaf(-c_low.u[row], c0, g) : fmaf(yk.na, c0, g);
+            VT g;
+            vld(Tc + i * TW, g);
+            cn = LOW ? vfma(-c_low.u[row], c0, g) : vfma(yk.na, c0, g);
+        } else if (row == -1) {
+            cn = vext(c0, c1);
         } else {
-            cn = (row == -1) ? fmaf(2.0f, c0, -c1) : 0.f;
+            vzero(cn);
         }
         c3 = c2; c2 = c1; c1 = c0; c0 = cn;
-        if (FINAL && i == CH - 2) c2 = fmaf(2.0f, c1, -c0);
+        if (FINAL && i == CH - 2) c2 = vext(c1, c0);
         if (i == CH - 1) n1 = c0;
         if (i == CH - 2) n2 = c0;
         if (i == CH - 3) n3 = c0;
         if (i <= IEMIT) emit<FULL>(yk, ptr, row + 1, c0, c1, c2, c3);
     }
-    if (LOW && a == 0) s1 = fmaf(2.0f, c0, -c1);           // c'[-1] when row 0 opens the chunk
+    if (LOW && a == 0) s1 = vext(c0, c1);                  // c'[-1] when row 0 opens the chunk
     emit<FULL>(yk, ptr, a, s1, c0, c1, c2);
     emit<FULL>(yk, ptr, a - 1, s2, s1, c0, c1);
     emit<FULL>(yk, ptr, a - 2, s3, s2, s1, c0);
@@ -210,8 +246,8 @@ __device__ __forceinline__ void sweep(const float* Tc, int a, float cstart, cons
 
 // block-uniform dispatch: FULL when every interval the sweep evaluates (a-2 .. top) is stored
 template <bool LOW, bool FINAL>
-__device__ __forceinline__ void sweep_any(const float* Tc, int a, float cstart, const YK& yk, int kA, int kB, float& s1,
-                                          float& s2, float& s3)
+__device__ __forceinline__ void sweep_any(const float* Tc, int a, VT cstart, const YK& yk, int kA, int kB, VT& s1, VT& s2,
+                                          VT& s3)
 {
     const int ktop = a + (FINAL ? CH - 2 : CH - 3);
     if (a - 2 >= kA && ktop <= kB) sweep<LOW, FINAL, true>(Tc, a, cstart, yk, s1, s2, s3);
@@ -220,28 +256,30 @@ __device__ __forceinline__ void sweep_any(const float* Tc, int a, float cstart, 
 
 // Causal pass of one chunk in place (T -> g) and the look-ahead sum A = c'[a] seen from the chunk before.
 template <bool LOW>
-__device__ __forceinline__ float causal(float* Tc, int a, bool is_final, float na, float& gprev)
+__device__ __forceinline__ VT causal(float* Tc, int a, bool is_final, float na, VT& gprev)
 {
     constexpr PowTab PW = make_pow();
     const float inv6a = 1.0f / (6.0f * U_INF);
-    float A = 0.f, om = 1.f;
+    VT A;
+    vzero(A);
+    float om = 1.f;
 #pragma unroll
     for (int i = 0; i < CH; ++i) {
         const int row = a + i;
         if (LOW && row < 0) continue;                       // block-uniform
-        const float t = Tc[i * TW];
-        float g;
+        VT t, g;
+        vld(Tc + i * TW, t);
         if (LOW) {
             const float u = c_low.u[row];
-            g = fmaf(-u, gprev, c_low.p[row] * t);
-            A = fmaf(om, g, A);
+            g = vfma(-u, gprev, vmul(c_low.p[row], t));
+            A = vfma(om, g, A);
             om *= -u;
         } else {
-            g = fmaf(na, gprev, t);
-            A = fmaf(PW.v[i], g, A);
+            g = vfma(na, gprev, t);
+            A = vfma(PW.v[i], g, A);
         }
         gprev = g;
-        Tc[i * TW] = (i == CH - 1 && is_final) ? t * inv6a : g;      // last row of the plane: c'[h-1] = f[h-1] / 6a
+        vst(Tc + i * TW, (i == CH - 1 && is_final) ? vmul(inv6a, t) : g);     // last row of the plane: c'[h-1] = f[h-1] / 6a
     }
     return A;
 }
@@ -400,9 +438,9 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
         const float scx = sg.ax.ident ? 1.f : 6.0f * U_INF;
         const float wx[4] = {scx * sg.ax.w[0], scx * sg.ax.w[1], scx * sg.ax.w[2], scx * sg.ax.w[3]};
         const bool edge = sg.pL >= 0 || sg.pR >= 0;
-        // y-pass constants of this thread's column
-        const int col = sg.Xs + tid;
-        bool ycol = tid < TW && col < sg.Xe;
+        // y-pass constants of this thread's CY columns
+        const int col = sg.Xs + CY * tid;
+        bool ycol = CY * tid < TW && col < sg.Xe;           // Xe - Xs is a multiple of 4: a pair never straddles the strip's end
         YK yk;
         yk.na = -U_INF;
         const float scy = sg.ay.ident ? 1.f : 6.0f * U_INF;
@@ -410,12 +448,19 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
         yk.my = sg.ay.m; yk.ylo = sg.ylo; yk.yhi = sg.yhi;
         yk.po = outk + (ycol ? col : sg.Xs);
         yk.w = w;
-        if (ycol && !(col >= sg.ax.lo && col <= sg.ax.hi)) {
-            // a column outside the x footprint: fill, for every row of the segment that carries data; nothing else to do
-            for (int y = sg.ylo; y <= sg.yhi; ++y) yk.po[(size_t)((unsigned)y * (unsigned)w)] = fill;
-            ycol = false;
+        yk.in0 = col >= sg.ax.lo && col <= sg.ax.hi;
+        yk.in1 = CY == 2 ? (col + 1 >= sg.ax.lo && col + 1 <= sg.ax.hi) : yk.in0;
+        if (ycol && !(yk.in0 && yk.in1)) {
+            // columns outside the x footprint: fill, for every row of the segment that carries data
+            for (int y = sg.ylo; y <= sg.yhi; ++y) {
+                float* q = yk.po + (size_t)((unsigned)y * (unsigned)w);
+                if (!yk.in0) q[0] = fill;
+                if (CY == 2 && !yk.in1) q[1] = fill;
+            }
+            if (!yk.in0 && !yk.in1) ycol = false;            // nothing else to do for this thread
         }
-        float gprev = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+        VT gprev, s1, s2, s3;
+        vzero(gprev); vzero(s1); vzero(s2); vzero(s3);
 
         for (int j = 0; j < sg.nch; ++j) {
             const int a = sg.a0 + CH * j;                               // first source row of the chunk
@@ -472,24 +517,24 @@ k_resample_tile(const __grid_constant__ CUtensorMap tmap, int n, int w, int h, i
             }
             // ---------------- y pass: thread = column
             if (ycol) {
-                float* Tc = T + tid;
+                float* Tc = T + CY * tid;
                 if (sg.ay.ident) {
                     // pure row translation: interval k = source row k, weights (0, 1, 0, 0)
 #pragma unroll 4
                     for (int i = 0; i < CH; ++i) {
                         const int y = a + i - yk.my;
-                        if (y >= yk.ylo && y <= yk.yhi) yk.po[(size_t)((unsigned)y * (unsigned)w)] = Tc[i * TW];
+                        if (y >= yk.ylo && y <= yk.yhi) { VT t; vld(Tc + i * TW, t); put(yk, yk.po + (size_t)((unsigned)y * (unsigned)w), t); }
                     }
                 } else {
                     const bool is_final = a + CH == h;
                     const bool low = a <= CH;                            // rows < LOWROWS: tabulated coefficients
-                    const float A = low ? causal<true>(Tc, a, is_final, yk.na, gprev) : causal<false>(Tc, a, is_final, yk.na, gprev);
+                    const VT A = low ? causal<true>(Tc, a, is_final, yk.na, gprev) : causal<false>(Tc, a, is_final, yk.na, gprev);
                     if (j >= 1 && a - 1 >= sg.kA - 1) {                  // the chunk before holds rows that are evaluated
-                        const float* Tp = tring + ((j - 1) % NT) * T_FLOATS + tid;
+                        const float* Tp = tring + ((j - 1) % NT) * T_FLOATS + CY * tid;
                         if (a - CH <= CH) sweep_any<true, false>(Tp, a - CH, A, yk, sg.kA, sg.kB, s1, s2, s3);
                         else sweep_any<false, false>(Tp, a - CH, A, yk, sg.kA, sg.kB, s1, s2, s3);
                     }
-                    if (is_final && a + CH - 1 >= sg.kA - 1) sweep_any<false, true>(Tc, a, 0.f, yk, sg.kA, sg.kB, s1, s2, s3);
+                    if (is_final && a + CH - 1 >= sg.kA - 1) sweep_any<false, true>(Tc, a, A, yk, sg.kA, sg.kB, s1, s2, s3);
                 }
             }
             __syncthreads();                    // the next chunk has landed (seen by the last warp); with NT == 2 also: the
