@@ -181,3 +181,15 @@ def coadd(stack, footprint=None, mode=SIGCLIP, ksigma=3.0, max_iter=3, want64=Fa
     if rc:
         raise ValueError("orc_coadd: %d" % rc)
     return SimpleNamespace(out=out32, out64=out64, count=cnt, rejmask=mask, margin=margin)
+
+
+def fill_bad(frames, badmask):
+    """O7 (reading Q25): masked pixels replaced by linear interpolation along the short axis.  Returns a new array."""
+    out = np.array(_f32(frames), copy=True)
+    n, h, w = out.shape
+    badmask = np.ascontiguousarray(badmask, dtype=np.uint8)
+    assert badmask.shape == (h, w)
+    rc = lib().orc_fill_bad(_p(out, C.c_float), C.c_int(n), C.c_int(w), C.c_int(h), _p(badmask, C.c_uint8))
+    if rc:
+        raise ValueError("orc_fill_bad: %d" % rc)
+    return out

@@ -24,6 +24,7 @@
  *                       P5  SciPy natural CubicSpline, identity, integer shift, composition;
  *                       P6  round-trip magnitude vs the paper's printed 1e-2..1e-1 (L162, L225); P12 footprint
  *   orc_coadd           P8  identical frames; P9 one-outlier closed form; P10 Samuelson; P11 brute force
+ *   orc_fill_bad        P13 exact on linear ramps; clear mask = identity; dead row / hot column / corner rules; numpy brute force
  * Parity unpinned: equivalence with IRAF imshift / imcombine and accuracy of estimated
  * shifts against WCS astrometry (no IRAF, no MITSuME data in this environment).
  */
@@ -460,5 +461,58 @@ int orc_coadd(const float *stack, int n, int w, int h, const int32_t *footprint,
                     if (keep[i]) rejmask[(idx[i] / 32) * np + p] &= ~(1u << (idx[i] % 32));   /* ... minus the used */
             }
         }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7  bad-pixel fill ("bad pixel masking"; Table 6 L252 -- the step is named,
+ *     its rule is not; reading Q25 of DESIGN.md).  Every pixel with badmask != 0 is replaced by a
+ *     linear interpolation between the nearest GOOD pixels of the ORIGINAL frame (filled values are
+ *     never used as sources, so the result does not depend on an order):
+ *       xl < x < xr : nearest good pixels in the same row,  gap gx = xr - xl (infinite if one is missing)
+ *       yl < y < yu : nearest good pixels in the same column, gap gy = yu - yl
+ *       gx <= gy, finite : v = f[y][xl] + (f[y][xr] - f[y][xl]) (x - xl) / gx      (the short axis; ties -> x)
+ *       else gy finite   : v = f[yl][x] + (f[yu][x] - f[yl][x]) (y - yl) / gy
+ *       else             : the nearest of the one-sided neighbours (ties in the order xl, xr, yl, yu); none -> 0
+ *     A hot column is bridged across its two neighbours, a dead row across the rows above and below.
+ *     The mask is the same for every frame of the stack.  In place; float64 arithmetic, one rounding.
+ * ---------------------------------------------------------------------------------------- */
+int orc_fill_bad(float *frames, int n, int w, int h, const uint8_t *bad)
+{
+    if (n < 1 || w < 1 || h < 1 || !bad) return -1;
+    const size_t np = (size_t)w * h;
+    float *src = malloc(sizeof(float) * np);
+    for (int k = 0; k < n; ++k) {
+        float *f = frames + k * np;
+        memcpy(src, f, sizeof(float) * np);
+        for (int y = 0; y < h; ++y)
+            for (int x = 0; x < w; ++x) {
+                if (!bad[(size_t)y * w + x]) continue;
+                int xl = x - 1, xr = x + 1, yl = y - 1, yu = y + 1;
+                while (xl >= 0 && bad[(size_t)y * w + xl]) --xl;
+                while (xr < w && bad[(size_t)y * w + xr]) ++xr;
+                while (yl >= 0 && bad[(size_t)yl * w + x]) --yl;
+                while (yu < h && bad[(size_t)yu * w + x]) ++yu;
+                const int hx = xl >= 0 && xr < w, hy = yl >= 0 && yu < h;
+                double v = 0.0;
+                if (hx && (!hy || xr - xl <= yu - yl)) {
+                    double a = src[(size_t)y * w + xl], b = src[(size_t)y * w + xr];
+                    v = a + (b - a) * (double)(x - xl) / (double)(xr - xl);
+                } else if (hy) {
+                    double a = src[(size_t)yl * w + x], b = src[(size_t)yu * w + x];
+                    v = a + (b - a) * (double)(y - yl) / (double)(yu - yl);
+                } else {
+                    int best = -1, dist = 0;
+                    size_t at = 0;
+                    if (xl >= 0) { best = 0; dist = x - xl; at = (size_t)y * w + xl; }
+                    if (xr < w && (best < 0 || xr - x < dist)) { best = 1; dist = xr - x; at = (size_t)y * w + xr; }
+                    if (yl >= 0 && (best < 0 || y - yl < dist)) { best = 2; dist = y - yl; at = (size_t)yl * w + x; }
+                    if (yu < h && (best < 0 || yu - y < dist)) { best = 3; dist = yu - y; at = (size_t)yu * w + x; }
+                    v = best >= 0 ? (double)src[at] : 0.0;
+                }
+                f[(size_t)y * w + x] = (float)v;
+            }
+    }
+    free(src);
     return 0;
 }

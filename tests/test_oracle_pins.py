@@ -497,3 +497,76 @@ def test_end_to_end_oracle_recovers_truth():
     r = oracle.resample(c.out, -e.shift[:, 0], -e.shift[:, 1])
     o = oracle.coadd(r.out, r.footprint, mode=oracle.MEDIAN)
     assert abs(float(np.median(o.out)) - 1000.0) < 5.0
+
+
+# ---------------------------------------------------------------- P13 bad-pixel fill (O7, reading Q25)
+def _ramp(n, h, w):
+    yy, xx = np.mgrid[0:h, 0:w]
+    return np.stack([(100.0 + 3.0 * xx + 7.0 * yy + 11.0 * k) for k in range(n)]).astype(np.float32)
+
+
+def test_p13_fill_is_exact_on_linear_ramps_and_identity_without_mask():
+    """Linear interpolation along either axis reproduces a plane a + bx + cy exactly (integer values: no rounding), so
+    whatever axis and neighbours the rule picks, the filled frame equals the original; a clear mask changes nothing."""
+    n, h, w = 3, 24, 31
+    f = _ramp(n, h, w)
+    rng = np.random.default_rng(5)
+    bad = (rng.random((h, w)) < 0.15).astype(np.uint8)
+    bad[:, 9] = 1                     # hot column
+    bad[13, :] = 1                    # dead row
+    bad[3:6, 20:24] = 1               # cluster
+    bad[0, 0] = 1                     # corner: good neighbours on one side only in x and in y -> no interpolation
+    bad[0, 1] = 0; bad[1, 0] = 0
+    got = oracle.fill_bad(f, bad)
+    good = bad == 0
+    # pixels with good neighbours on BOTH sides along some axis are interpolated (exactly, on a plane); the others
+    # (image borders, the crossing of the dead row with the hot column) fall under the one-sided / none rules
+    left = np.maximum.accumulate(good, axis=1) & np.maximum.accumulate(good[:, ::-1], axis=1)[:, ::-1]
+    vert = np.maximum.accumulate(good, axis=0) & np.maximum.accumulate(good[::-1], axis=0)[::-1]
+    two_sided = good | left | vert
+    assert two_sided.mean() > 0.97 and not two_sided[13, 9] and not two_sided[0, 0]
+    assert np.array_equal(got[:, two_sided], f[:, two_sided])
+    assert np.array_equal(got[:, 0, 0], f[:, 0, 1])          # one-sided: the nearest (xr and yu both 1 away: order xl, xr, yl, yu)
+    assert np.all(got[:, 13, 9] == 0.0)                      # no good pixel in its row or its column: 0
+    noisy = rng.normal(1000, 30, size=(n, h, w)).astype(np.float32)
+    assert np.array_equal(oracle.fill_bad(noisy, np.zeros((h, w), np.uint8)), noisy)
+    assert np.array_equal(oracle.fill_bad(noisy, bad)[:, good], noisy[:, good])     # good pixels never change
+
+
+def test_p13_fill_rules_and_numpy_brute_force():
+    n, h, w = 2, 17, 23
+    rng = np.random.default_rng(6)
+    f = rng.normal(1000, 30, size=(n, h, w)).astype(np.float32)
+    bad = (rng.random((h, w)) < 0.2).astype(np.uint8)
+    bad[:, 5] = 1
+    bad[8, :] = 1
+    got = oracle.fill_bad(f, bad)
+    f64 = f.astype(np.float64)
+    # independent statement with numpy searches
+    for y in range(h):
+        for x in range(w):
+            if not bad[y, x]:
+                continue
+            gx = np.flatnonzero(bad[y] == 0)
+            gy = np.flatnonzero(bad[:, x] == 0)
+            xl = gx[gx < x].max() if (gx < x).any() else None
+            xr = gx[gx > x].min() if (gx > x).any() else None
+            yl = gy[gy < y].max() if (gy < y).any() else None
+            yu = gy[gy > y].min() if (gy > y).any() else None
+            hx, hy = xl is not None and xr is not None, yl is not None and yu is not None
+            if hx and (not hy or xr - xl <= yu - yl):
+                exp = f64[:, y, xl] + (f64[:, y, xr] - f64[:, y, xl]) * (x - xl) / (xr - xl)
+            elif hy:
+                exp = f64[:, yl, x] + (f64[:, yu, x] - f64[:, yl, x]) * (y - yl) / (yu - yl)
+            else:
+                cand = [(x - xl, 0, (y, xl)) if xl is not None else None, (xr - x, 1, (y, xr)) if xr is not None else None,
+                        (y - yl, 2, (yl, x)) if yl is not None else None, (yu - y, 3, (yu, x)) if yu is not None else None]
+                cand = [c for c in cand if c is not None]
+                exp = f64[:, cand and min(cand)[2][0], min(cand)[2][1]] if cand else np.zeros(n)
+            assert np.array_equal(got[:, y, x], exp.astype(np.float32)), (y, x)
+    # a hot column is bridged across its two neighbours; a dead row across the rows above and below (where those are good)
+    y, x = 3, 5
+    if not bad[y, 4] and not bad[y, 6]:
+        assert np.allclose(got[:, y, x], 0.5 * (f64[:, y, 4] + f64[:, y, 6]), rtol=0, atol=1e-4)
+    # everything masked -> 0
+    assert np.all(oracle.fill_bad(f, np.ones((h, w), np.uint8)) == 0.0)
