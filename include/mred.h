@@ -70,7 +70,8 @@ typedef enum {
     MRED_CALL_ESTIMATE_SHIFTS = 2,
     MRED_CALL_RESAMPLE = 3,
     MRED_CALL_COADD = 4,
-    MRED_CALL_REDUCE = 5
+    MRED_CALL_REDUCE = 5,
+    MRED_CALL_FILL_BAD = 6
 } mred_call;
 
 /*
@@ -98,6 +99,16 @@ int mred_build_masters(const mred_geom *geom, const uint16_t *bias, int nb, cons
 int mred_calibrate(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
                    const float *MD, const float *MF, float *out, double *level_out, void *ws, size_t ws_bytes,
                    void *stream);
+
+/*
+ * Bad-pixel fill ("bad pixel masking", Table 6; O7, reading Q25), in place on a float32
+ * stack, e.g. between mred_calibrate and mred_resample: every pixel with badmask != 0 becomes the linear interpolation
+ * between the nearest good pixels of the same frame along the axis with the shorter gap (ties: x), else the nearest
+ * one-sided good neighbour (order left, right, below, above), else 0.  Good pixels are never changed and filled values
+ * are never used as sources.  frames: float32 [n][h][w]; badmask: uint8 [h][w] (the same for every frame).
+ * 1 <= n <= 65535; ws: mred_workspace_bytes(MRED_CALL_FILL_BAD, ..) bytes (a list entry per pixel of the plane).
+ */
+int mred_fill_bad(float *frames, int n, int w, int h, const uint8_t *badmask, void *ws, size_t ws_bytes, void *stream);
 
 /*
  * Per-frame offset relative to frame `ref_index` from marginal profiles (O4; replaces

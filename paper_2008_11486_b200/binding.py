@@ -15,12 +15,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmred.so")
 
 MEDIAN, MEAN, SIGCLIP = 0, 1, 2
-CALL_BUILD_MASTERS, CALL_CALIBRATE, CALL_ESTIMATE_SHIFTS, CALL_RESAMPLE, CALL_COADD, CALL_REDUCE = range(6)
+CALL_BUILD_MASTERS, CALL_CALIBRATE, CALL_ESTIMATE_SHIFTS, CALL_RESAMPLE, CALL_COADD, CALL_REDUCE, CALL_FILL_BAD = range(7)
 MAX_STACK = 255
 
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
            "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
-           "mred_reduce_workspace_views",
+           "mred_reduce_workspace_views", "mred_fill_bad",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -155,6 +155,18 @@ def calibrate(g, raw, dark_scale, MB, MD, MF, out=None, level_out=None, ws=None,
                               C.c_size_t(ws.numel()), _stream(stream))
     _check(rc, "mred_calibrate")
     return out, level_out
+
+
+def fill_bad(frames, badmask, ws=None, stream=None):
+    """include/mred.h: mred_fill_bad.  In place on `frames` (float32 [n][h][w]); returns it."""
+    n, h, w = frames.shape
+    _shape(badmask, (h, w), "badmask")
+    ws = _ws(ws, workspace_bytes(CALL_FILL_BAD, Geom(0, 0, 0, 0, 0, 0, w, h), n), frames.device)
+    rc = lib().mred_fill_bad(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
+                             _dev(badmask, torch.uint8, "badmask"), C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()),
+                             _stream(stream))
+    _check(rc, "mred_fill_bad")
+    return frames
 
 
 def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stream=None):

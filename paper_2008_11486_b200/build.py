@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmred.so")
-SOURCES = ["api.cu", "calibrate.cu", "coadd.cu", "masters.cu", "estimate.cu", "resample.cu"]
+SOURCES = ["api.cu", "calibrate.cu", "coadd.cu", "masters.cu", "estimate.cu", "resample.cu", "fill.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]

@@ -135,6 +135,7 @@ size_t mred_workspace_bytes(int call, const mred_geom* geom, int n)
         case MRED_CALL_RESAMPLE: return resample_ws_bytes(g.w, g.h, n);   /* optional: without it the one-kernel route runs */
         case MRED_CALL_COADD: return 0;
         case MRED_CALL_REDUCE: return carve_reduce(nullptr, g, n).bytes;
+        case MRED_CALL_FILL_BAD: return fill_ws_bytes(g.w, g.h);
         default: return 0;
     }
 }
@@ -175,6 +176,15 @@ int mred_calibrate(const mred_geom* geom, const uint16_t* raw, int n, float dark
     int rc = launch_frame_sums(raw, g, n, os, nullptr, 0, st);
     if (rc) return rc;
     return launch_calibrate(raw, g, n, dark_scale, MB, MD, MF, out, level_out, os, st);
+}
+
+int mred_fill_bad(float* frames, int n, int w, int h, const uint8_t* badmask, void* ws, size_t ws_bytes, void* stream)
+{
+    if (!frames || !badmask || n < 1 || n > 65535 || w < 1 || h < 1) return MRED_EINVAL;
+    if ((int64_t)w * h >= (int64_t)1 << 31) return MRED_EINVAL;
+    if (!aligned16(frames) || !aligned16(badmask)) return MRED_EALIGN;
+    if (!ws || !aligned16(ws) || ws_bytes < fill_ws_bytes(w, h)) return MRED_EWORKSPACE;
+    return launch_fill_bad(frames, n, w, h, badmask, ws, static_cast<cudaStream_t>(stream));
 }
 
 int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index, int max_lag,

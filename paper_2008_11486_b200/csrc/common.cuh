@@ -140,5 +140,7 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
                     const double* dshift_dev /* [n][2] (dx,dy): shift = -d */, float fill, float* out,
                     int32_t* fp_dev /* nullable */, void* ws /* nullable */, size_t ws_bytes, cudaStream_t st);
 size_t resample_ws_bytes(int w, int h, int n);
+int launch_fill_bad(float* frames, int n, int w, int h, const uint8_t* bad, void* ws, cudaStream_t st);
+size_t fill_ws_bytes(int w, int h);
 
 }  // namespace mred

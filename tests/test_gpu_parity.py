@@ -660,6 +660,53 @@ def test_estimate_shifts_tie_rule():
     assert np.array_equal(host(plan.shift), e.shift)
 
 
+# ------------------------------------------------------------------ NEXT-1: bad-pixel fill (O7)
+def test_fill_bad_parity_and_rules():
+    """mred_fill_bad against oracle.fill_bad: random masks with a hot column, a dead row, clusters, masked borders and a
+    fully masked plane; good pixels bit-identical, filled ones at the stated bar; exact on a plane a + bx + cy."""
+    rng = np.random.default_rng(21)
+    for (n, h, w, dens) in ((3, 61, 131, 0.15), (2, 136, 192, 0.02), (5, 40, 64, 0.5)):
+        f = rng.normal(1000, 30, size=(n, h, w)).astype(np.float32)
+        bad = (rng.random((h, w)) < dens).astype(np.uint8)
+        bad[:, 7] = 1
+        bad[h // 2, :] = 1
+        bad[3:7, 20:25] = 1
+        bad[0, :3] = 1
+        bad[:, w - 1] = 1
+        ref = oracle.fill_bad(f, bad)
+        got = host(mred.fill_bad(dev(f), dev(bad)))
+        good = bad == 0
+        assert np.array_equal(got[:, good], f[:, good])
+        assert_close(got, ref, "fill_bad %dx%d" % (h, w))
+    yy, xx = np.mgrid[0:50, 0:70]
+    plane = np.stack([(100.0 + 3.0 * xx + 7.0 * yy + 5.0 * k) for k in range(2)]).astype(np.float32)
+    bad = (rng.random((50, 70)) < 0.2).astype(np.uint8)
+    bad[0, :] = 0; bad[-1, :] = 0; bad[:, 0] = 0; bad[:, -1] = 0       # every masked pixel has both neighbours along an axis
+    assert np.array_equal(host(mred.fill_bad(dev(plane), dev(bad))), plane)
+    ones = np.ones((40, 64), np.uint8)
+    assert np.all(host(mred.fill_bad(dev(f), dev(ones))) == 0.0)
+    clear = np.zeros((40, 64), np.uint8)
+    assert np.array_equal(host(mred.fill_bad(dev(f), dev(clear))), f)
+
+
+def test_fill_bad_config4_full_size():
+    """Config 4's real hot-column mask at full size: calibrate -> fill on the GPU against the oracle's calibrate -> fill;
+    after the fill the hot columns no longer stand out, so estimate_shifts finds the same shifts WITHOUT the mask."""
+    grp = synth.make_group(4, n_sci=8, n_master=3)
+    g = grp.geom
+    m = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat)
+    c = oracle.calibrate(g, grp.sci, 1.0, m.MB, m.MD, m.MF)
+    ref = oracle.fill_bad(c.out, grp.badmask)
+    out, _ = mred.calibrate(g, dev(grp.sci), 1.0, dev(m.MB), dev(m.MD), dev(m.MF))
+    mred.fill_bad(out, dev(grp.badmask))
+    assert_close(host(out), ref, "calibrate + fill, config 4")
+    e_mask = oracle.estimate_shifts(c.out, 0, 16, badmask=grp.badmask)
+    ish, sh = mred.estimate_shifts(out, 0, 16)                       # no mask: the filled frames
+    e_fill = oracle.estimate_shifts(ref, 0, 16)
+    assert np.array_equal(host(ish), e_fill.ishift) and np.max(np.abs(host(sh) - e_fill.shift)) <= 1e-3
+    assert np.array_equal(e_fill.ishift, e_mask.ishift)               # the fill does what the mask did
+
+
 # ------------------------------------------------------------------ error behaviour
 def test_error_codes():
     g = GEOMS["small"]
