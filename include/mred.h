@@ -178,6 +178,16 @@ int mred_reduce_staged(const mred_geom *geom, const uint16_t *raw, int n, float 
                        void *const *events);
 
 /*
+ * mred_reduce with the bad-pixel fill (mred_fill_bad, O7) applied to the calibrated stack before it is
+ * resampled: calibrate -> estimate_shifts (masked pixels left out of the profiles) -> fill -> resample -> coadd.
+ * badmask must not be NULL.  Same workspace as mred_reduce.
+ */
+int mred_reduce_filled(const mred_geom *geom, const uint16_t *raw, int n, float dark_scale, const float *MB,
+                       const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
+                       float fill, const mred_comb_opts *opts, float *out, uint16_t *count, uint32_t *rejmask,
+                       double *shift_out, int32_t *footprint_out, void *ws, size_t ws_bytes, void *stream);
+
+/*
  * Same as mred_reduce with HOST input and output buffers: raw_host (uint16 [n][H][W], ideally
  * pinned) is copied to the device inside the call, out_host (float32 [h][w]), count_host
  * (uint16 [h][w], nullable) and shift_host (float64 [n][2], nullable) are copied back; all on

@@ -17,7 +17,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mred_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-MEDIAN, MEAN, SIGCLIP = 0, 1, 2
+MEDIAN, MEAN, SIGCLIP, MINMAX = 0, 1, 2, 3
+SPLINE, BILINEAR, NEAREST = 0, 1, 2
+PARABOLA, GAUSSIAN = 0, 1
 
 
 def build(force: bool = False) -> str:
@@ -115,7 +117,7 @@ def calibrate(geom, raw, dark_scale, MB, MD, MF, want64=False):
     return SimpleNamespace(out=out32, out64=out64, level=lev)
 
 
-def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None):
+def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, peak=PARABOLA):
     frames = _f32(frames)
     n, h, w = frames.shape
     if badmask is not None:
@@ -123,9 +125,9 @@ def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None):
         assert badmask.shape == (h, w)
     ish = np.zeros((n, 2), np.int32)
     sh = np.zeros((n, 2), np.float64)
-    rc = lib().orc_estimate_shifts(_p(frames, C.c_float), C.c_int(n), C.c_int(w), C.c_int(h),
-                                   C.c_int(ref_index), C.c_int(max_lag), _p(badmask, C.c_uint8),
-                                   _p(ish, C.c_int32), _p(sh, C.c_double))
+    rc = lib().orc_estimate_shifts_peak(_p(frames, C.c_float), C.c_int(n), C.c_int(w), C.c_int(h),
+                                        C.c_int(ref_index), C.c_int(max_lag), _p(badmask, C.c_uint8), C.c_int(peak),
+                                        _p(ish, C.c_int32), _p(sh, C.c_double))
     if rc:
         raise ValueError("orc_estimate_shifts: %d" % rc)
     return SimpleNamespace(ishift=ish, shift=sh)
@@ -137,7 +139,7 @@ def footprint(w, h, sx, sy):
     return fp
 
 
-def resample(frames, sx, sy, fill=0.0, want64=False):
+def resample(frames, sx, sy, fill=0.0, want64=False, interp=SPLINE):
     frames = _f32(frames)
     n, h, w = frames.shape
     sx = np.ascontiguousarray(np.broadcast_to(np.asarray(sx, np.float64), (n,)))
@@ -145,9 +147,9 @@ def resample(frames, sx, sy, fill=0.0, want64=False):
     out32 = np.empty((n, h, w), np.float32)
     out64 = np.empty((n, h, w), np.float64) if want64 else None
     fp = np.zeros((n, 4), np.int32)
-    rc = lib().orc_resample(_p(frames, C.c_float), C.c_int(n), C.c_int(w), C.c_int(h),
-                            _p(sx, C.c_double), _p(sy, C.c_double), C.c_double(fill),
-                            _p(out64, C.c_double), _p(out32, C.c_float), _p(fp, C.c_int32))
+    rc = lib().orc_resample_interp(_p(frames, C.c_float), C.c_int(n), C.c_int(w), C.c_int(h),
+                                   _p(sx, C.c_double), _p(sy, C.c_double), C.c_double(fill), C.c_int(interp),
+                                   _p(out64, C.c_double), _p(out32, C.c_float), _p(fp, C.c_int32))
     if rc:
         raise ValueError("orc_resample: %d" % rc)
     return SimpleNamespace(out=out32, out64=out64, footprint=fp)

@@ -39,7 +39,7 @@ typedef struct {
     int32_t x0, y0, w, h;  /* image rectangle kept by the overscan cutout (L63)               */
 } orc_geom;
 
-enum { ORC_MEDIAN = 0, ORC_MEAN = 1, ORC_SIGCLIP = 2 };
+enum { ORC_MEDIAN = 0, ORC_MEAN = 1, ORC_SIGCLIP = 2, ORC_MINMAX = 3 };
 
 /* ------------------------------------------------------------------------------------------
  * O1  overscan ("pedestal") level: per-frame mean of the overscan pixels,
@@ -86,6 +86,16 @@ static double combine_column(const double *v, int m, int mode, double ksigma, in
     unsigned char alive[256];
     for (int i = 0; i < m; ++i) alive[i] = 1;
     int n = m;
+    if (mode == ORC_MINMAX && m >= 3) {
+        /* NEXT-2 variant (IRAF imcombine "minmax" with nlow = nhigh = 1; reading Q26): leave out one minimum and one
+         * maximum (the first occurrence of each in frame order, the maximum among the entries other than the dropped
+         * minimum), mean of the rest.  Fewer than 3 values: plain mean. */
+        int imin = 0, imax = -1;
+        for (int i = 1; i < m; ++i) if (v[i] < v[imin]) imin = i;
+        for (int i = 0; i < m; ++i) if (i != imin && (imax < 0 || v[i] > v[imax])) imax = i;
+        alive[imin] = 0; alive[imax] = 0;
+        n = m - 2;
+    }
     if (mode == ORC_SIGCLIP) {
         for (int it = 0; it < max_iter && n > 0; ++it) {
             double mu = 0.0, var = 0.0;
@@ -265,7 +275,7 @@ static void profiles(const float *f, int w, int h, const uint8_t *bad, double *p
     free(cx); free(cy);
 }
 
-static void best_lag(const double *a, const double *b, int n, int R, int32_t *il, double *fl)
+static void best_lag(const double *a, const double *b, int n, int R, int peak, int32_t *il, double *fl)
 {
     double *C = malloc(sizeof(double) * (2 * R + 1));
     for (int l = -R; l <= R; ++l) {
@@ -282,6 +292,12 @@ static void best_lag(const double *a, const double *b, int n, int R, int32_t *il
     if (abs(best) < R) {
         double cm = C[best - 1 + R], c0 = C[best + R], cp = C[best + 1 + R];
         double den = cm - 2.0 * c0 + cp;
+        if (peak == 1 && cm > 0.0 && c0 > 0.0 && cp > 0.0) {
+            /* NEXT-2 variant (reading Q27): the parabola through the LOGARITHMS of the three samples, exact for a
+             * Gaussian correlation peak; the plain parabola where a sample is not positive */
+            cm = log(cm); c0 = log(c0); cp = log(cp);
+            den = cm - 2.0 * c0 + cp;
+        }
         if (den < 0.0) {
             delta = 0.5 * (cm - cp) / den;
             if (delta > 0.5) delta = 0.5;
@@ -293,8 +309,18 @@ static void best_lag(const double *a, const double *b, int n, int R, int32_t *il
     free(C);
 }
 
+int orc_estimate_shifts_peak(const float *frames, int n, int w, int h, int ref_index, int max_lag,
+                             const uint8_t *badmask, int peak, int32_t *ishift, double *shift);
+
 int orc_estimate_shifts(const float *frames, int n, int w, int h, int ref_index, int max_lag,
                         const uint8_t *badmask, int32_t *ishift, double *shift)
+{
+    return orc_estimate_shifts_peak(frames, n, w, h, ref_index, max_lag, badmask, 0, ishift, shift);
+}
+
+/* peak: 0 = 3-point parabola (O4 v), 1 = 3-point parabola of the logarithms (Gaussian peak, NEXT-2) */
+int orc_estimate_shifts_peak(const float *frames, int n, int w, int h, int ref_index, int max_lag,
+                             const uint8_t *badmask, int peak, int32_t *ishift, double *shift)
 {
     if (n < 1 || ref_index < 0 || ref_index >= n || max_lag < 0) return -1;
     const size_t np = (size_t)w * h;
@@ -304,8 +330,8 @@ int orc_estimate_shifts(const float *frames, int n, int w, int h, int ref_index,
     for (int k = 0; k < n; ++k) {
         if (k == ref_index) { ishift[2 * k] = ishift[2 * k + 1] = 0; shift[2 * k] = shift[2 * k + 1] = 0.0; continue; }
         profiles(frames + k * np, w, h, badmask, bx, by);
-        best_lag(ax, bx, w, max_lag, &ishift[2 * k], &shift[2 * k]);
-        best_lag(ay, by, h, max_lag, &ishift[2 * k + 1], &shift[2 * k + 1]);
+        best_lag(ax, bx, w, max_lag, peak, &ishift[2 * k], &shift[2 * k]);
+        best_lag(ay, by, h, max_lag, peak, &ishift[2 * k + 1], &shift[2 * k + 1]);
     }
     free(ax); free(ay); free(bx); free(by);
     return 0;
@@ -361,16 +387,32 @@ static double spline_eval(const double *c /* as above */, int n, double uu)
 }
 
 /* one axis of `len` samples with stride 1 in `f`; writes out[i] and ok[i] */
-static void shift_axis(const double *f, int len, double s, double *out, unsigned char *ok, double *cbuf)
+static void shift_axis_interp(const double *f, int len, double s, int interp, double *out, unsigned char *ok, double *cbuf)
 {
     int integer = (s == floor(s));
-    if (!integer) spline_coeffs(f, len, cbuf);
+    if (!integer && interp == 0) spline_coeffs(f, len, cbuf);
     for (int i = 0; i < len; ++i) {
         double uu = (double)i - s;
         ok[i] = (uu >= 0.0 && uu <= (double)(len - 1));
         if (!ok[i]) { out[i] = 0.0; continue; }
-        out[i] = integer ? f[(int)uu] : spline_eval(cbuf, len, uu);
+        if (integer) out[i] = f[(int)uu];
+        else if (interp == 0) out[i] = spline_eval(cbuf, len, uu);
+        else if (interp == 1) {                  /* NEXT-2: linear interpolation, no prefilter */
+            int k = (int)floor(uu);
+            if (k > len - 2) k = len - 2;
+            double t = uu - (double)k;
+            out[i] = (1.0 - t) * f[k] + t * f[k + 1];
+        } else {                                 /* nearest neighbour: floor(u + 1/2) */
+            int j = (int)floor(uu + 0.5);
+            if (j > len - 1) j = len - 1;
+            out[i] = f[j];
+        }
     }
+}
+
+static void shift_axis(const double *f, int len, double s, double *out, unsigned char *ok, double *cbuf)
+{
+    shift_axis_interp(f, len, s, 0, out, ok, cbuf);
 }
 
 void orc_footprint(int w, int h, double sx, double sy, int32_t *fp)
@@ -383,8 +425,19 @@ void orc_footprint(int w, int h, double sx, double sy, int32_t *fp)
     fp[3] = b < (double)(h - 1) ? (b < -1.0 ? -1 : (int32_t)b) : h - 1;
 }
 
+int orc_resample_interp(const float *in, int n, int w, int h, const double *sx, const double *sy, double fill, int interp,
+                        double *out64, float *out32, int32_t *footprint);
+
 int orc_resample(const float *in, int n, int w, int h, const double *sx, const double *sy, double fill,
                  double *out64, float *out32, int32_t *footprint)
+{
+    return orc_resample_interp(in, n, w, h, sx, sy, fill, 0, out64, out32, footprint);
+}
+
+/* interp: 0 = natural bicubic spline (O5), 1 = bilinear, 2 = nearest neighbour (NEXT-2; same shift sense, validity and
+ * footprint; an axis with an integer shift is a copy in every variant) */
+int orc_resample_interp(const float *in, int n, int w, int h, const double *sx, const double *sy, double fill, int interp,
+                        double *out64, float *out32, int32_t *footprint)
 {
     if (n < 1 || w < 2 || h < 2) return -1;
     const size_t np = (size_t)w * h;
@@ -397,12 +450,12 @@ int orc_resample(const float *in, int n, int w, int h, const double *sx, const d
         if (footprint) orc_footprint(w, h, sx[k], sy[k], footprint + 4 * k);
         for (int y = 0; y < h; ++y) {                    /* rows first */
             for (int x = 0; x < w; ++x) line[x] = (double)f[(size_t)y * w + x];
-            shift_axis(line, w, sx[k], res, okx, cbuf);
+            shift_axis_interp(line, w, sx[k], interp, res, okx, cbuf);
             for (int x = 0; x < w; ++x) T[(size_t)y * w + x] = res[x];
         }
         for (int x = 0; x < w; ++x) {                    /* then columns */
             for (int y = 0; y < h; ++y) line[y] = T[(size_t)y * w + x];
-            shift_axis(line, h, sy[k], res, oky, cbuf);
+            shift_axis_interp(line, h, sy[k], interp, res, oky, cbuf);
             for (int y = 0; y < h; ++y) {
                 double v = (okx[x] && oky[y]) ? res[y] : fill;
                 if (out64) out64[k * np + (size_t)y * w + x] = v;

@@ -20,7 +20,7 @@ MAX_STACK = 255
 
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
            "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
-           "mred_reduce_workspace_views", "mred_fill_bad",
+           "mred_reduce_workspace_views", "mred_fill_bad", "mred_reduce_filled",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -283,11 +283,23 @@ def _reduce_shapes(plan, raw, MB, MD, MF, badmask):
 
 
 def reduce(plan: ReducePlan, raw, dark_scale, MB, MD, MF, ref_index=0, max_lag=32, badmask=None, fill=0.0,
-           mode=SIGCLIP, ksigma=3.0, max_iter=3, stream=None, events=None):
+           mode=SIGCLIP, ksigma=3.0, max_iter=3, stream=None, events=None, fill_bad=False):
     """include/mred.h: mred_reduce / mred_reduce_staged (device-resident chained science path).  Results land
     in `plan`.  events: optional list of 5 torch.cuda.Event(enable_timing=True) recorded around the stages."""
     _reduce_shapes(plan, raw, MB, MD, MF, badmask)
     o = _opts(mode, ksigma, max_iter)
+    if fill_bad:       # include/mred.h: mred_reduce_filled (no stage events)
+        if badmask is None or events is not None:
+            raise MredError("fill_bad needs a badmask and takes no stage events")
+        rc = lib().mred_reduce_filled(C.byref(plan.g), _dev(raw, torch.uint16, "raw"), C.c_int(plan.n), C.c_float(dark_scale),
+                           _dev(MB, torch.float32, "MB"), _dev(MD, torch.float32, "MD"), _dev(MF, torch.float32, "MF"),
+                           C.c_int(ref_index), C.c_int(max_lag), _dev(badmask, torch.uint8, "badmask"),
+                           C.c_float(fill), C.byref(o), _dev(plan.out, torch.float32, "out"),
+                           _dev(plan.count, torch.uint16, "count"), _dev(plan.mask, torch.uint32, "rejmask"),
+                           _dev(plan.shift, torch.float64, "shift"), _dev(plan.footprint, torch.int32, "footprint"),
+                           C.c_void_p(plan.ws.data_ptr()), C.c_size_t(plan.ws.numel()), _stream(stream))
+        _check(rc, "mred_reduce_filled")
+        return plan
     ev = C.c_void_p(None)
     if events is not None:
         for e in events:

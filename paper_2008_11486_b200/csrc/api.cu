@@ -40,6 +40,7 @@ struct ReduceWs {
     void* est;                // estimate workspace
     void* rs;                 // resample workspace (x-shifted stack, small stacks only)
     size_t rs_bytes;
+    void* fill;               // list of the bad-pixel fill (mred_reduce_filled)
     size_t bytes;
 };
 
@@ -58,6 +59,7 @@ static ReduceWs carve_reduce(void* ws, const Geom& g, int n)
     r.est = take(estimate_ws_bytes(g.w, g.h, n));
     r.rs_bytes = resample_ws_bytes(g.w, g.h, n);
     r.rs = take(r.rs_bytes);
+    r.fill = take(fill_ws_bytes(g.w, g.h));
     r.bytes = (size_t)(p - static_cast<char*>(ws));
     return r;
 }
@@ -242,12 +244,12 @@ int mred_reduce_workspace_views(const mred_geom* geom, int n, size_t* calibrated
     return MRED_OK;
 }
 
-int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+static int reduce_impl(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
                        const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
                        const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
-                       int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream, void* const* events)
+                       int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream, void* const* events, bool fill_bad)
 {
-    if (!raw || !out) return MRED_EINVAL;
+    if (!raw || !out || (fill_bad && !badmask)) return MRED_EINVAL;
     if (!aligned16(raw) || !aligned16(out)) return MRED_EALIGN;
     int rc = reduce_args_ok(geom, n, MB, MD, MF, ref_index, max_lag, badmask, opts, count, rejmask, shift_out, footprint_out);
     if (rc) return rc;
@@ -277,12 +279,33 @@ int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float 
     int32_t* fp = footprint_out ? footprint_out : r.fp;
     if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, est_flags, st))) return rc;
     MRED_STAGE_EVENT(2);
+    // bad-pixel fill (O7) between the calibrated stack and its resampling: a hot pixel would otherwise ring through the
+    // spline prefilter; the profile sums above were taken without the masked pixels, so the shifts do not depend on it
+    if (fill_bad && (rc = launch_fill_bad(r.cal, n, g.w, g.h, badmask, r.fill, st))) return rc;
     if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, r.rs, r.rs_bytes, st))) return rc;
     MRED_STAGE_EVENT(3);
     if ((rc = launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st))) return rc;
     MRED_STAGE_EVENT(4);
 #undef MRED_STAGE_EVENT
     return MRED_OK;
+}
+
+int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+                       const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                       const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
+                       int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream, void* const* events)
+{
+    return reduce_impl(geom, raw, n, dark_scale, MB, MD, MF, ref_index, max_lag, badmask, fill, opts, out, count, rejmask,
+                       shift_out, footprint_out, ws, ws_bytes, stream, events, false);
+}
+
+int mred_reduce_filled(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
+                       const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                       const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
+                       int32_t* footprint_out, void* ws, size_t ws_bytes, void* stream)
+{
+    return reduce_impl(geom, raw, n, dark_scale, MB, MD, MF, ref_index, max_lag, badmask, fill, opts, out, count, rejmask,
+                       shift_out, footprint_out, ws, ws_bytes, stream, nullptr, true);
 }
 
 int mred_reduce(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,

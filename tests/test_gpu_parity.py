@@ -358,7 +358,7 @@ def test_resample_bspline_image_matches_paper_precision(golden):
 CHAIN_MARGIN = 0.05      # ADU: clip decisions closer than this to the threshold are not compared in the chained path (Q20)
 
 
-def _chain_check(grp, max_lag, mode, what, resample_frames=None):
+def _chain_check(grp, max_lag, mode, what, resample_frames=None, fill_bad=False):
     """mred_reduce (the device-chained path bench.py times) against the oracle, stage by stage on the SAME upstream
     data, so that every float comparison is at the stated bar (no loose percentile bound):
       masters   mred_build_masters vs oracle (strict);
@@ -381,7 +381,10 @@ def _chain_check(grp, max_lag, mode, what, resample_frames=None):
     e = oracle.estimate_shifts(c.out, 0, max_lag, badmask=grp.badmask)
     plan = mred.ReducePlan(g, n, want_mask=True)
     bad = dev(grp.badmask) if grp.badmask is not None else None
-    mred.reduce(plan, dev(grp.sci), scale, dev(m.MB), dev(m.MD), dev(m.MF), 0, max_lag, badmask=bad, mode=mode)
+    mred.reduce(plan, dev(grp.sci), scale, dev(m.MB), dev(m.MD), dev(m.MF), 0, max_lag, badmask=bad, mode=mode,
+                fill_bad=fill_bad)
+    if fill_bad:       # mred_reduce_filled: the calibrated stack is filled in place (O7) before it is resampled
+        c.out = oracle.fill_bad(c.out, grp.badmask)
     assert_close(host(plan.calibrated()), c.out, what + " calibrated stack (k_calibrate_prof)")
     sh = host(plan.shift)
     assert np.max(np.abs(sh - e.shift)) <= 1e-3, np.max(np.abs(sh - e.shift))
@@ -504,6 +507,15 @@ def test_config4_full_size_chained_with_badmask():
     assert grp.badmask is not None and grp.badmask.any()
     e, _ = _chain_check(grp, 16, 2, "config 4", resample_frames=(1, 17, 40, 63))
     assert np.max(np.abs(e.shift - grp.shifts)) < 0.5          # diagnostic (Q10: cosmic rays cost accuracy)
+
+
+def test_reduce_filled_chain():
+    """mred_reduce_filled: the chained path with the bad-pixel fill between calibrate and resample, against the oracle chain
+    calibrate -> estimate (mask) -> fill -> resample -> coadd; small geometry and config 4 at full size (24 frames)."""
+    grp = synth.make_group(4, geom=synth.GEOM_SMALL, stars=30, S=6.0, n_sci=24, n_master=4)
+    _chain_check(grp, 12, 2, "small config 4, filled", fill_bad=True)
+    grp = synth.make_group(4, n_sci=24, n_master=4)
+    _chain_check(grp, 16, 2, "config 4 (24 frames), filled", resample_frames=(1, 11, 23), fill_bad=True)
 
 
 def test_config5_large_format_chained():

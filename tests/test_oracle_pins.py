@@ -570,3 +570,80 @@ def test_p13_fill_rules_and_numpy_brute_force():
         assert np.allclose(got[:, y, x], 0.5 * (f64[:, y, 4] + f64[:, y, 6]), rtol=0, atol=1e-4)
     # everything masked -> 0
     assert np.all(oracle.fill_bad(f, np.ones((h, w), np.uint8)) == 0.0)
+
+
+# ---------------------------------------------------------------- P14-P16 NEXT-2 variants (readings Q26-Q28)
+def test_p14_minmax_rejection_closed_forms_and_brute_force():
+    """minmax (one lowest, one highest left out): values 1..N -> mean of 2..N-1 = (N+1)/2, count N-2, the mask names the
+    frames of the minimum and the maximum; N identical frames -> that frame (the two dropped ones are the first two);
+    fewer than 3 values -> plain mean; random columns against numpy's sorted[1:-1].mean()."""
+    for n in (3, 4, 10, 33):
+        st = np.arange(1, n + 1, dtype=np.float32)[::-1].copy().reshape(n, 1, 1)      # frame k holds N - k
+        o = oracle.coadd(st, None, mode=oracle.MINMAX)
+        assert o.out64 is None and o.out[0, 0] == np.float32((n + 1) / 2.0) and o.count[0, 0] == n - 2
+        bits = sum(int(o.rejmask[wd, 0, 0]) << (32 * wd) for wd in range(o.rejmask.shape[0]))
+        assert bits == (1 << (n - 1)) | 1                     # frame N-1 holds the minimum 1, frame 0 the maximum N
+    same = np.full((5, 2, 2), 7.25, np.float32)
+    o = oracle.coadd(same, None, mode=oracle.MINMAX)
+    assert np.all(o.out == 7.25) and np.all(o.count == 3) and np.all(o.rejmask[0] == 0b00011)
+    two = np.array([3.0, 9.0], np.float32).reshape(2, 1, 1)
+    o = oracle.coadd(two, None, mode=oracle.MINMAX)
+    assert o.out[0, 0] == 6.0 and o.count[0, 0] == 2 and o.rejmask[0, 0, 0] == 0
+    rng = np.random.default_rng(14)
+    st = rng.normal(1000, 30, size=(17, 8, 8)).astype(np.float32)
+    o = oracle.coadd(st, None, mode=oracle.MINMAX, want64=True)
+    exp = np.sort(st.astype(np.float64), axis=0)[1:-1].mean(axis=0)
+    np.testing.assert_allclose(o.out64, exp, rtol=1e-13)
+
+
+def test_p15_gaussian_peak_is_exact_for_gaussian_profiles():
+    """The log-parabola through three samples of a Gaussian has its vertex at the Gaussian's centre: for frames whose
+    profiles are Gaussians the GAUSSIAN peak fit returns the injected sub-pixel shift, where the plain parabola is off by
+    thousandths to hundredths of a pixel (test_p7_subpixel_parabola_closed_form).  Integer part and tie rule are shared."""
+    w, h = 96, 80
+    x, y = np.arange(w), np.arange(h)
+
+    def fr(cx, cy):
+        px = np.exp(-0.5 * ((x - cx) / 3.0) ** 2)
+        py = np.exp(-0.5 * ((y - cy) / 3.0) ** 2)
+        return (100.0 * py[:, None] + 100.0 * px[None, :]).astype(np.float32)
+    fs = np.stack([fr(46.0, 40.0), fr(48.3, 38.6), fr(44.55, 41.2)])
+    g = oracle.estimate_shifts(fs, 0, 10, peak=oracle.GAUSSIAN)
+    p = oracle.estimate_shifts(fs, 0, 10, peak=oracle.PARABOLA)
+    truth = np.array([[0, 0], [2.3, -1.4], [-1.45, 1.2]])
+    assert np.array_equal(g.ishift, p.ishift) and np.array_equal(g.ishift, np.rint(truth).astype(np.int32))
+    assert np.max(np.abs(g.shift - truth)) < 2e-4, np.max(np.abs(g.shift - truth))
+    assert np.max(np.abs(p.shift - truth)) > 1e-3            # the parabola's bias (2.7e-3 px here), for contrast
+    assert np.all(g.shift[0] == 0.0)
+
+
+def test_p16_bilinear_and_nearest_resampling():
+    """bilinear: exact on a plane a + bx + cy for any shift; equals scipy.ndimage.shift(order=1) away from the borders;
+    t = 1/2 is the mean of the two neighbours.  nearest: a shift s is the integer translation by floor(s + 1/2) ... of the
+    source index floor(x - s + 1/2).  Integer shifts are copies in both; footprints as for the spline."""
+    from scipy import ndimage
+    h, w = 40, 52
+    yy, xx = np.mgrid[0:h, 0:w]
+    plane = (10.0 + 3.0 * xx + 7.0 * yy).astype(np.float32)
+    sx, sy = 2.25, -1.5
+    r = oracle.resample(plane[None], [sx], [sy], fill=-1.0, want64=True, interp=oracle.BILINEAR)
+    fp = r.footprint[0]
+    sl = (slice(fp[2], fp[3] + 1), slice(fp[0], fp[1] + 1))
+    exp = 10.0 + 3.0 * (xx - sx) + 7.0 * (yy - sy)
+    assert np.array_equal(r.out64[0][sl], exp[sl])
+    assert np.all(r.out64[0][:, :fp[0]] == -1.0) and np.array_equal(fp, oracle.resample(plane[None], [sx], [sy]).footprint[0])
+    rng = np.random.default_rng(16)
+    img = rng.normal(1000, 30, size=(h, w)).astype(np.float32)
+    r = oracle.resample(img[None], [0.3], [1.7], want64=True, interp=oracle.BILINEAR)
+    ref = ndimage.shift(img.astype(np.float64), (1.7, 0.3), order=1, mode="constant", cval=0.0, prefilter=False)
+    np.testing.assert_allclose(r.out64[0][3:-3, 3:-3], ref[3:-3, 3:-3], rtol=1e-12, atol=1e-9)
+    half = oracle.resample(img[None], [0.5], [0.0], want64=True, interp=oracle.BILINEAR).out64[0]
+    np.testing.assert_allclose(half[:, 1:], 0.5 * (img[:, 1:].astype(np.float64) + img[:, :-1]), rtol=1e-15)
+    for s, k in ((2.3, 2), (2.5, 2), (2.7, 3), (-0.4, 0), (-0.6, -1)):          # source index floor(x - s + 1/2) = x - k
+        nn = oracle.resample(img[None], [s], [0.0], interp=oracle.NEAREST)
+        lo, hi = nn.footprint[0][0], nn.footprint[0][1]
+        cols = np.arange(lo, hi + 1)
+        assert np.array_equal(nn.out[0][:, cols], img[:, cols - k]), (s, k)
+    for interp in (oracle.BILINEAR, oracle.NEAREST):
+        r = oracle.resample(img[None], [3.0], [-2.0], fill=0.0, interp=interp)
+        assert np.array_equal(r.out[0][0:h - 2, 3:], img[2:, :w - 3])
