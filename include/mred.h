@@ -48,7 +48,9 @@ typedef struct {
     int32_t x0, y0, w, h; /* image rectangle kept by the overscan cutout               */
 } mred_geom;
 
-typedef enum { MRED_MEDIAN = 0, MRED_MEAN = 1, MRED_SIGCLIP = 2 } mred_combine;
+typedef enum { MRED_MEDIAN = 0, MRED_MEAN = 1, MRED_SIGCLIP = 2, MRED_MINMAX = 3 /* mred_coadd only */ } mred_combine;
+typedef enum { MRED_PEAK_PARABOLA = 0, MRED_PEAK_GAUSSIAN = 1 } mred_peak;
+typedef enum { MRED_INTERP_SPLINE = 0, MRED_INTERP_BILINEAR = 1, MRED_INTERP_NEAREST = 2 } mred_interp;
 
 typedef struct {
     int32_t mode;     /* mred_combine                                                             */
@@ -125,6 +127,16 @@ int mred_estimate_shifts(const float *frames, int n, int w, int h, int ref_index
                          void *stream);
 
 /*
+ * mred_estimate_shifts with a choice of the sub-pixel estimator (Q27): peak =
+ * MRED_PEAK_PARABOLA is mred_estimate_shifts; MRED_PEAK_GAUSSIAN fits the parabola to the LOGARITHMS of the three
+ * correlation samples around the maximum (exact for a Gaussian peak), and falls back to the plain parabola where one of
+ * them is not positive.  Integer part, tie rule and everything else are unchanged.
+ */
+int mred_estimate_shifts_peak(const float *frames, int n, int w, int h, int ref_index, int max_lag,
+                              const uint8_t *badmask, int peak, int32_t *ishift, double *shift, void *ws,
+                              size_t ws_bytes, void *stream);
+
+/*
  * Sub-pixel shift by bicubic (tensor-product natural cubic) spline interpolation (PAPER.md L63,
  * L107, L164, L266; O5):  out_k(x, y) = spline_k(x - sx[k], y - sy[k]); pixels whose
  * source lies outside the frame get `fill`.  An axis whose shift has zero fractional part is a
@@ -141,13 +153,25 @@ int mred_resample(const float *in, int n, int w, int h, const double *sx, const 
                   float *out, int32_t *footprint, void *ws, size_t ws_bytes, void *stream);
 
 /*
+ * mred_resample with a choice of the interpolator (PAPER.md L239 suggests cheaper ones; Q28):
+ * MRED_INTERP_SPLINE is mred_resample (without workspace); MRED_INTERP_BILINEAR takes the two nearest source samples per axis
+ * with weights (1 - t, t), MRED_INTERP_NEAREST the sample floor(u + 1/2), u = x - sx; no prefilter.  Shift sense, validity
+ * (0 <= u <= n - 1 on both axes, else `fill`), footprint and the bit-exact copy for integer shifts are those of the spline.
+ * sx, sy, footprint: HOST.  w, h >= 2.
+ */
+int mred_resample_interp(const float *in, int n, int w, int h, const double *sx, const double *sy, float fill,
+                         int interp, float *out, int32_t *footprint, void *stream);
+
+/*
  * Per-pixel combine along the stack axis (O6) over the
  * frames whose footprint contains the pixel: median, mean, or ksigma-clipped mean (mean-centred,
  * population sigma, keep |v-mu| <= k sigma, <= max_iter passes, early stop).
  * stack: float32 [n][h][w]; footprint: HOST int32 [n][4] (nullable = every frame covers every
  * pixel); out: float32 [h][w]; count: uint16 [h][w] number of frames used (nullable);
  * rejmask: uint32 [ceil(n/32)][h][w], bit k%32 of word k/32 set iff frame k was NOT used
- * (nullable).  No covering frame -> value 0, count 0.
+ * (nullable).  No covering frame -> value 0, count 0.  mode MRED_MINMAX (Q26; mred_coadd and
+ * mred_reduce* only): the mean without one minimum and one maximum (first occurrences in frame order; fewer than 3 values:
+ * the plain mean).
  */
 int mred_coadd(const float *stack, int n, int w, int h, const int32_t *footprint, const mred_comb_opts *opts,
                float *out, uint16_t *count, uint32_t *rejmask, void *stream);

@@ -14,13 +14,15 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmred.so")
 
-MEDIAN, MEAN, SIGCLIP = 0, 1, 2
+MEDIAN, MEAN, SIGCLIP, MINMAX = 0, 1, 2, 3
+PEAK_PARABOLA, PEAK_GAUSSIAN = 0, 1
+INTERP_SPLINE, INTERP_BILINEAR, INTERP_NEAREST = 0, 1, 2
 CALL_BUILD_MASTERS, CALL_CALIBRATE, CALL_ESTIMATE_SHIFTS, CALL_RESAMPLE, CALL_COADD, CALL_REDUCE, CALL_FILL_BAD = range(7)
 MAX_STACK = 255
 
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
            "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
-           "mred_reduce_workspace_views", "mred_fill_bad", "mred_reduce_filled",
+           "mred_reduce_workspace_views", "mred_fill_bad", "mred_reduce_filled", "mred_estimate_shifts_peak", "mred_resample_interp",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -169,7 +171,7 @@ def fill_bad(frames, badmask, ws=None, stream=None):
     return frames
 
 
-def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stream=None):
+def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stream=None, peak=0):
     """include/mred.h: mred_estimate_shifts.  Returns (ishift int32 [n][2], shift float64 [n][2]) on device."""
     n, h, w = frames.shape
     dev = frames.device
@@ -178,10 +180,10 @@ def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stre
     _shape(badmask, (h, w), "badmask")
     gg = Geom(0, 0, 0, 0, 0, 0, w, h)
     ws = _ws(ws, workspace_bytes(CALL_ESTIMATE_SHIFTS, gg, n), dev)
-    rc = lib().mred_estimate_shifts(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
-                                    C.c_int(ref_index), C.c_int(max_lag), _dev(badmask, torch.uint8, "badmask"),
-                                    _dev(ish, torch.int32, "ishift"), _dev(sh, torch.float64, "shift"),
-                                    C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream(stream))
+    rc = lib().mred_estimate_shifts_peak(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
+                                         C.c_int(ref_index), C.c_int(max_lag), _dev(badmask, torch.uint8, "badmask"),
+                                         C.c_int(peak), _dev(ish, torch.int32, "ishift"), _dev(sh, torch.float64, "shift"),
+                                         C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream(stream))
     _check(rc, "mred_estimate_shifts")
     return ish, sh
 
@@ -208,6 +210,23 @@ def resample(frames, sx, sy, fill=0.0, out=None, ws=None, stream=None):
                              C.c_void_p(ws.data_ptr() if ws is not None else None),
                              C.c_size_t(ws.numel() if ws is not None else 0), _stream(stream))
     _check(rc, "mred_resample")
+    return out, fp
+
+
+def resample_interp(frames, sx, sy, interp, fill=0.0, out=None, stream=None):
+    """include/mred.h: mred_resample_interp (bilinear / nearest / spline).  Returns (out, footprint int32 [n][4] numpy)."""
+    n, h, w = frames.shape
+    sx = np.ascontiguousarray(np.broadcast_to(np.asarray(sx, np.float64), (n,)))
+    sy = np.ascontiguousarray(np.broadcast_to(np.asarray(sy, np.float64), (n,)))
+    if out is None:
+        out = torch.empty_like(frames)
+    _shape(out, (n, h, w), "out")
+    fp = np.zeros((n, 4), np.int32)
+    rc = lib().mred_resample_interp(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
+                                    sx.ctypes.data_as(C.c_void_p), sy.ctypes.data_as(C.c_void_p), C.c_float(fill),
+                                    C.c_int(interp), _dev(out, torch.float32, "out"), fp.ctypes.data_as(C.c_void_p),
+                                    _stream(stream))
+    _check(rc, "mred_resample_interp")
     return out, fp
 
 

@@ -22,10 +22,11 @@ int sm_count()
     return n;
 }
 
-static bool opts_ok(const mred_comb_opts* o)
+static bool opts_ok(const mred_comb_opts* o, bool allow_minmax = false)
 {
     if (!o) return false;
-    if (o->mode != MRED_MEDIAN && o->mode != MRED_MEAN && o->mode != MRED_SIGCLIP) return false;
+    if (o->mode != MRED_MEDIAN && o->mode != MRED_MEAN && o->mode != MRED_SIGCLIP && !(allow_minmax && o->mode == MRED_MINMAX))
+        return false;
     if (o->mode == MRED_SIGCLIP && (!(o->ksigma >= 0.f) || o->max_iter < 0)) return false;
     return true;
 }
@@ -92,7 +93,7 @@ static int reduce_args_ok(const mred_geom* geom, int n, const float* MB, const f
                           int max_lag, const uint8_t* badmask, const mred_comb_opts* opts, const uint16_t* count,
                           const uint32_t* rejmask, const double* shift_out, const int32_t* footprint_out)
 {
-    if (!geom_ok(geom) || !MB || !MD || !MF || !opts_ok(opts)) return MRED_EINVAL;
+    if (!geom_ok(geom) || !MB || !MD || !MF || !opts_ok(opts, true)) return MRED_EINVAL;
     if (n < 1 || n > MRED_MAX_STACK || geom->w < 4 || geom->h < 4 || geom->w > MRED_MAX_PROFILE || geom->h > MRED_MAX_PROFILE)
         return MRED_EINVAL;
     if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= geom->w || max_lag >= geom->h)
@@ -189,19 +190,28 @@ int mred_fill_bad(float* frames, int n, int w, int h, const uint8_t* badmask, vo
     return launch_fill_bad(frames, n, w, h, badmask, ws, static_cast<cudaStream_t>(stream));
 }
 
-int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index, int max_lag,
-                         const uint8_t* badmask, int32_t* ishift, double* shift, void* ws, size_t ws_bytes,
-                         void* stream)
+int mred_estimate_shifts_peak(const float* frames, int n, int w, int h, int ref_index, int max_lag,
+                              const uint8_t* badmask, int peak, int32_t* ishift, double* shift, void* ws, size_t ws_bytes,
+                              void* stream)
 {
     if (!frames || !ishift || !shift || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1) return MRED_EINVAL;
     if (w > MRED_MAX_PROFILE || h > MRED_MAX_PROFILE) return MRED_EINVAL;   // a whole profile is sorted in shared memory
     if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= w || max_lag >= h)
         return MRED_EINVAL;
+    if (peak != MRED_PEAK_PARABOLA && peak != MRED_PEAK_GAUSSIAN) return MRED_EINVAL;
     if (!aligned16(frames) || !aligned16(ishift) || !aligned16(shift) || (badmask && !aligned16(badmask)))
         return MRED_EALIGN;
     if (!ws || !aligned16(ws) || ws_bytes < estimate_ws_bytes(w, h, n)) return MRED_EWORKSPACE;
-    return launch_estimate(frames, n, w, h, ref_index, max_lag, badmask, ishift, shift, ws, 0,
+    return launch_estimate(frames, n, w, h, ref_index, max_lag, badmask, ishift, shift, ws, 0, peak,
                            static_cast<cudaStream_t>(stream));
+}
+
+int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index, int max_lag,
+                         const uint8_t* badmask, int32_t* ishift, double* shift, void* ws, size_t ws_bytes,
+                         void* stream)
+{
+    return mred_estimate_shifts_peak(frames, n, w, h, ref_index, max_lag, badmask, MRED_PEAK_PARABOLA, ishift, shift, ws,
+                                     ws_bytes, stream);
 }
 
 int mred_resample(const float* in, int n, int w, int h, const double* sx, const double* sy, float fill,
@@ -223,10 +233,31 @@ int mred_resample(const float* in, int n, int w, int h, const double* sx, const 
     return launch_resample(in, n, w, h, sx, sy, nullptr, fill, out, nullptr, ws, ws_bytes, static_cast<cudaStream_t>(stream));
 }
 
+int mred_resample_interp(const float* in, int n, int w, int h, const double* sx, const double* sy, float fill,
+                         int interp, float* out, int32_t* footprint, void* stream)
+{
+    if (interp == MRED_INTERP_SPLINE) return mred_resample(in, n, w, h, sx, sy, fill, out, footprint, nullptr, 0, stream);
+    if (interp != MRED_INTERP_BILINEAR && interp != MRED_INTERP_NEAREST) return MRED_EINVAL;
+    if (!in || !out || !sx || !sy || n < 1 || n > MRED_MAX_STACK || w < 2 || h < 2 || in == out) return MRED_EINVAL;
+    if ((int64_t)w * h >= (int64_t)1 << 31) return MRED_EINVAL;
+    for (int k = 0; k < n; ++k)
+        if (!isfinite(sx[k]) || !isfinite(sy[k]) || fabs(sx[k]) > 1.0e6 || fabs(sy[k]) > 1.0e6) return MRED_EINVAL;
+    if (!aligned16(in) || !aligned16(out)) return MRED_EALIGN;
+    if (footprint)
+        for (int k = 0; k < n; ++k) {
+            int lo, hi;
+            axis_footprint(w, sx[k], lo, hi);
+            footprint[4 * k] = lo; footprint[4 * k + 1] = hi;
+            axis_footprint(h, sy[k], lo, hi);
+            footprint[4 * k + 2] = lo; footprint[4 * k + 3] = hi;
+        }
+    return launch_resample_lin(in, n, w, h, sx, sy, interp, fill, out, static_cast<cudaStream_t>(stream));
+}
+
 int mred_coadd(const float* stack, int n, int w, int h, const int32_t* footprint, const mred_comb_opts* opts,
                float* out, uint16_t* count, uint32_t* rejmask, void* stream)
 {
-    if (!stack || !out || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1 || !opts_ok(opts)) return MRED_EINVAL;
+    if (!stack || !out || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1 || !opts_ok(opts, true)) return MRED_EINVAL;
     if ((int64_t)w * h >= (int64_t)1 << 31) return MRED_EINVAL;
     if (!aligned16(stack) || !aligned16(out) || (count && !aligned16(count)) || (rejmask && !aligned16(rejmask)))
         return MRED_EALIGN;
@@ -277,7 +308,7 @@ static int reduce_impl(const mred_geom* geom, const uint16_t* raw, int n, float 
     MRED_STAGE_EVENT(1);
     double* shift = shift_out ? shift_out : r.shift;
     int32_t* fp = footprint_out ? footprint_out : r.fp;
-    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, est_flags, st))) return rc;
+    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, est_flags, MRED_PEAK_PARABOLA, st))) return rc;
     MRED_STAGE_EVENT(2);
     // bad-pixel fill (O7) between the calibrated stack and its resampling: a hot pixel would otherwise ring through the
     // spline prefilter; the profile sums above were taken without the masked pixels, so the shifts do not depend on it

@@ -163,6 +163,23 @@ __global__ void __launch_bounds__(128) k_coadd_any(const float* __restrict__ sta
                 if (rank == ib) b = v[i];
             }
             value = 0.5f * a + 0.5f * b;
+        } else if (MODE == MRED_MINMAX) {
+            // one minimum and one maximum (first occurrences) left out, mean of the rest; fewer than 3 values: plain mean
+            float sum = 0.f, mn = CUDART_INF_F, mx = -CUDART_INF_F;
+            int imn = -1, imx = -1;
+            for (int k = 0; k < n; ++k)
+                if (used[k]) { sum += v[k]; if (v[k] < mn) { mn = v[k]; imn = k; } if (v[k] > mx) { mx = v[k]; imx = k; } }
+            if (m >= 3) {
+                if (imx == imn) { imx = -1; for (int k = 0; k < n && imx < 0; ++k) if (used[k] && k != imn) imx = k; }
+                const float c = sum / (float)m;
+                float r1 = 0.f;
+                for (int k = 0; k < n; ++k) if (used[k]) r1 += v[k] - c;
+                value = c + ((r1 - (mn - c)) - (mx - c)) / (float)(m - 2);
+                used[imn] = 0; used[imx] = 0;
+                cnt = m - 2;
+            } else {
+                value = sum / (float)m;
+            }
         } else {
             float sum = 0.f;
             for (int k = 0; k < n; ++k) if (used[k]) sum += v[k];
@@ -247,7 +264,12 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
         const cuuint32_t box[2] = {(cuuint32_t)cs::TPS, (cuuint32_t)n};
         if (!tma::encode_f32_map(&tm, stack, 2, dims, strides, box)) { set_cuda_error(cudaErrorInvalidValue); return MRED_ECUDA; }
         k_coadd_stream<<<dim3((unsigned)((np + cs::TP - 1) / cs::TP)), cs::TP, (size_t)n * cs::TPS * 4, st>>>(
-            tm, n, w, h, fpd, use_fp, local, o.mode == MRED_SIGCLIP ? 1 : 0, ks, mi, out, count, rejmask);
+            tm, n, w, h, fpd, use_fp, local, o.mode, ks, mi, out, count, rejmask);
+        MRED_LAUNCH_CHECK();
+        return MRED_OK;
+    }
+    if (o.mode == MRED_MINMAX) {       // planes whose size is not a multiple of 4: the any-N kernel
+        k_coadd_any<MRED_MINMAX><<<dim3((unsigned)((np + 127) / 128)), 128, 0, st>>>(stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
         MRED_LAUNCH_CHECK();
         return MRED_OK;
     }

@@ -144,7 +144,7 @@ __device__ __forceinline__ void clip_dirty(const ClipArgs& a, int tid)
 // grid (ceil(np / 128)), block 128, dynamic shared memory n * 528 bytes; tmap: dims {w*h, n}, box {132, n}
 __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__ CUtensorMap tmap, int n, int w, int h,
                                                          const int4* __restrict__ fp_dev, int use_fp,
-                                                         const __grid_constant__ HostFootprints hfp, int clip, float ksigma,
+                                                         const __grid_constant__ HostFootprints hfp, int mode, float ksigma,
                                                          int max_iter, float* __restrict__ out, uint16_t* __restrict__ count,
                                                          uint32_t* __restrict__ rejmask)
 {
@@ -203,7 +203,8 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__
     const size_t p = p0 + tid;
     float* col = vals + tid;
     const bool fast = s_nall == n;                          // block-uniform: every frame covers every pixel of the tile
-    const bool do_clip = clip && max_iter > 0;
+    const bool do_clip = mode == MRED_SIGCLIP && max_iter > 0;
+    const bool minmax = mode == MRED_MINMAX;
     const int words = (n + 31) >> 5;
     // one warp polls the mbarrier, the others sleep at the block barrier (128 polling threads took a fifth of all issue
     // slots away from the blocks that had their data); the barrier carries the copies' visibility on to them
@@ -227,7 +228,36 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__
                 if (!ok) col[k * TPS] = CUDART_NAN_F;
             }
         }
-        if (!do_clip) {
+        bool nan_marks = !fast;              // the column holds NaN marks (absent frames, minmax rejects) for the mask
+        if (minmax) {
+            // NEXT-2 variant (Q26): one minimum and one maximum (first occurrences in frame order) are left out,
+            // mean of the rest; fewer than 3 values: plain mean.  Compensated like the plain mean below.
+            float sum = 0.f, mn = CUDART_INF_F, mx = -CUDART_INF_F;
+            int imn = -1, imx = -1;
+            for (int k = 0; k < n; ++k) {
+                const float v = col[k * TPS];
+                if (!(v == v)) continue;
+                sum += v; ++m;
+                if (v < mn) { mn = v; imn = k; }
+                if (v > mx) { mx = v; imx = k; }
+            }
+            if (m >= 3) {
+                if (imx == imn) {            // every value equal: the maximum is the first entry other than the minimum
+                    imx = -1;
+                    for (int k = 0; k < n && imx < 0; ++k) { const float v = col[k * TPS]; if (v == v && k != imn) imx = k; }
+                }
+                const float c = sum / (float)m;
+                float r1 = 0.f;
+                for (int k = 0; k < n; ++k) { const float d = col[k * TPS] - c; if (d == d) r1 += d; }
+                value = c + ((r1 - (mn - c)) - (mx - c)) / (float)(m - 2);
+                col[imn * TPS] = CUDART_NAN_F;
+                col[imx * TPS] = CUDART_NAN_F;
+                m -= 2;
+                nan_marks = true;
+            } else if (m > 0) {
+                value = sum / (float)m;
+            }
+        } else if (!do_clip) {
             // plain mean, compensated: the sum, then the sum of the residuals about the float32 mean (what the first
             // sum lost to rounding next to a 60000-ADU outlier comes back with the second)
             float sum = 0.f;
@@ -297,7 +327,7 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__
             if (rejmask) {
                 for (int wd = 0; wd < words; ++wd) {
                     uint32_t bits = 0u;
-                    if (!fast) {
+                    if (nan_marks) {
                         const int k0 = 32 * wd, k1 = min(n, k0 + 32);
                         for (int k = k0; k < k1; ++k) { const float v = col[k * TPS]; if (!(v == v)) bits |= 1u << (k - k0); }
                     }

@@ -132,7 +132,7 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
 enum { EST_ZEROED = 1, EST_HAVE_SUMS = 2, EST_SHARED_COUNTS = 4 };   // 4: valid-pixel counts of the mask in frame 0's arrays (launch_mask_counts)
 int launch_mask_counts(const uint8_t* bad, int w, int h, int n, void* ws, cudaStream_t st);
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
-                    int32_t* ishift, double* shift, void* ws, int flags, cudaStream_t st);
+                    int32_t* ishift, double* shift, void* ws, int flags, int peak /* 0 parabola, 1 log-parabola */, cudaStream_t st);
 size_t estimate_ws_bytes(int w, int h, int n);
 // the accumulators inside an estimate workspace: what has to be zero before the sums start, and where they are
 void estimate_accumulators(void* ws, int w, int h, int n, void** zero, size_t* zero_bytes, long long** colsum, long long** rowsum);
@@ -140,6 +140,8 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
                     const double* dshift_dev /* [n][2] (dx,dy): shift = -d */, float fill, float* out,
                     int32_t* fp_dev /* nullable */, void* ws /* nullable */, size_t ws_bytes, cudaStream_t st);
 size_t resample_ws_bytes(int w, int h, int n);
+int launch_resample_lin(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host, int interp,
+                        float fill, float* out, cudaStream_t st);
 int launch_fill_bad(float* frames, int n, int w, int h, const uint8_t* bad, void* ws, cudaStream_t st);
 size_t fill_ws_bytes(int w, int h);
 

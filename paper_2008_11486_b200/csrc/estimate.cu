@@ -275,7 +275,7 @@ __global__ void __launch_bounds__(1024) k_finalize(int w, int h, int has_bad, Es
 // memory, lags dealt round-robin to the warps of the CORR_Z blocks; the last block of a (frame, axis) to finish
 // takes the argmax (ties: smaller |l|, then smaller l) and the 3-point parabola.
 constexpr int CORR_Z = 8;
-__global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref, int R, EstimateWs e,
+__global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref, int R, int peak, EstimateWs e,
                                                    int32_t* __restrict__ ishift, double* __restrict__ shift)
 {
     extern __shared__ double s_dyn[];     // a[len], b[len]
@@ -321,7 +321,8 @@ __global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref,
     double delta = 0.0;
     const int ab = best < 0 ? -best : best;
     if (ab < R) {
-        const double cm = sC[best - 1 + R], c0 = sC[best + R], cp = sC[best + 1 + R];
+        double cm = sC[best - 1 + R], c0 = sC[best + R], cp = sC[best + 1 + R];
+        if (peak == 1 && cm > 0.0 && c0 > 0.0 && cp > 0.0) { cm = log(cm); c0 = log(c0); cp = log(cp); }   // Gaussian peak (Q27)
         const double den = cm - 2.0 * c0 + cp;
         if (den < 0.0) {
             delta = 0.5 * (cm - cp) / den;
@@ -341,7 +342,7 @@ int launch_mask_counts(const uint8_t* bad, int w, int h, int n, void* ws, cudaSt
 }
 
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
-                    int32_t* ishift, double* shift, void* ws, int flags, cudaStream_t st)
+                    int32_t* ishift, double* shift, void* ws, int flags, int peak, cudaStream_t st)
 {
     const EstimateWs e = carve_est(ws, w, h, n);
     const int vec_ok = (w % 4 == 0) ? 1 : 0;
@@ -361,7 +362,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     }
     k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, bad ? ((flags & EST_SHARED_COUNTS) ? 2 : 1) : 0, e);
     MRED_LAUNCH_CHECK();
-    k_correlate<<<dim3(n, 2, CORR_Z), 256, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, e, ishift, shift);
+    k_correlate<<<dim3(n, 2, CORR_Z), 256, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, peak, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }

@@ -88,6 +88,7 @@ __device__ __forceinline__ Axis make_axis(int n, double s)
 #include "resample_warp.cuh"
 #include "resample_ypass.cuh"
 #include "resample_tile.cuh"
+#include "resample_lin.cuh"
 
 namespace mred {
 
@@ -158,6 +159,17 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
     const int strips = (w + OUTCOLS - 1) / OUTCOLS;
     const int BH = band_rows((long long)strips * n, h);
     k_resample<0><<<dim3(strips, (h + BH - 1) / BH, n), 32, smem, st>>>(in, n, w, h, hs, dshift_dev, fill, out, fpd, BH, vec);
+    MRED_LAUNCH_CHECK();
+    return MRED_OK;
+}
+
+int launch_resample_lin(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host, int interp,
+                        float fill, float* out, cudaStream_t st)
+{
+    HostShifts hs;
+    for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
+    const size_t np = (size_t)w * h;
+    k_resample_lin<<<dim3((unsigned)((np + 255) / 256), (unsigned)n), 256, 0, st>>>(in, w, h, hs, interp, fill, out);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }

@@ -719,6 +719,67 @@ def test_fill_bad_config4_full_size():
     assert np.array_equal(e_fill.ishift, e_mask.ishift)               # the fill does what the mask did
 
 
+# ------------------------------------------------------------------ NEXT-2 variants
+@pytest.mark.parametrize("n", [1, 2, 3, 10, 33, 64, 100])
+@pytest.mark.parametrize("aligned", [False, True])
+def test_coadd_minmax_parity(n, aligned):
+    """MRED_MINMAX (one minimum and one maximum left out): value at the stated bar, count and mask bit-exact (the frames that
+    hold the extremes are unique on continuous data), with footprints; streaming kernel (aligned) and any-N kernel."""
+    h, w = (60, 132) if aligned else (61, 131)
+    st, fp = _stack(n, h, w, 300 + n)
+    ref = oracle.coadd(st, fp, mode=oracle.MINMAX)
+    out, cnt, mask = mred.coadd(dev(st), fp, mode=mred.MINMAX, want_mask=True)
+    assert np.array_equal(host(cnt), ref.count)
+    assert np.array_equal(host(mask), ref.rejmask)
+    assert_close(host(out), ref.out, "coadd minmax n %d" % n)
+    same = np.repeat(st[:1], max(n, 3), axis=0)                       # all equal: the first two frames are the ones dropped
+    o2, c2, m2 = mred.coadd(dev(same), None, mode=mred.MINMAX, want_mask=True)
+    r2 = oracle.coadd(same, None, mode=oracle.MINMAX)
+    assert np.array_equal(host(c2), r2.count) and np.array_equal(host(m2), r2.rejmask) and np.array_equal(host(o2), r2.out)
+
+
+def test_estimate_shifts_gaussian_peak():
+    """MRED_PEAK_GAUSSIAN against the oracle on a star field (within 1e-3 px, integer part identical) and on Gaussian
+    profiles, where it recovers the injected sub-pixel shift itself."""
+    grp, m, c = _calibrated_small(stars=30, S=9.0, n_sci=6)
+    ref = oracle.estimate_shifts(c.out, 0, 24, peak=oracle.GAUSSIAN)
+    ish, sh = mred.estimate_shifts(dev(c.out), 0, 24, peak=mred.PEAK_GAUSSIAN)
+    assert np.array_equal(host(ish), ref.ishift) and np.max(np.abs(host(sh) - ref.shift)) <= 1e-3
+    w, h = 96, 80
+    x, y = np.arange(w), np.arange(h)
+    fr = lambda cx, cy: (100.0 * np.exp(-0.5 * ((y - cy) / 3.0) ** 2)[:, None] + 100.0 * np.exp(-0.5 * ((x - cx) / 3.0) ** 2)[None, :]).astype(np.float32)
+    fs = np.stack([fr(46.0, 40.0), fr(48.3, 38.6), fr(44.55, 41.2)])
+    ish, sh = mred.estimate_shifts(dev(fs), 0, 10, peak=mred.PEAK_GAUSSIAN)
+    assert np.max(np.abs(host(sh) - np.array([[0, 0], [2.3, -1.4], [-1.45, 1.2]]))) < 2e-4
+
+
+@pytest.mark.parametrize("interp", [1, 2])
+@pytest.mark.parametrize("shape", [(136, 192), (71, 183), (300, 420)])
+def test_resample_interp_parity(shape, interp):
+    """mred_resample_interp (bilinear, nearest) against the oracle: footprints bit-exact, values at the stated bar (nearest:
+    bit-exact copies), integer shifts copies, zero shift the identity; interp = spline routes to mred_resample."""
+    h, w = shape
+    rng = np.random.default_rng(h + w + interp)
+    n = len(SHIFTS)
+    img = rng.normal(1000, 30, size=(n, h, w)).astype(np.float32)
+    img[rng.random(img.shape) < 0.005] = 65535.0
+    sx = np.array([s[0] for s in SHIFTS])
+    sy = np.array([s[1] for s in SHIFTS])
+    ref = oracle.resample(img, sx, sy, fill=-5.0, interp=interp)
+    out, fp = mred.resample_interp(dev(img), sx, sy, interp, fill=-5.0)
+    got = host(out)
+    assert np.array_equal(fp, ref.footprint)
+    if interp == 2:
+        assert np.array_equal(got, ref.out)
+    else:
+        assert_close(got, ref.out, "bilinear %s" % (shape,))
+    assert np.array_equal(got[0], img[0])
+    if interp == 1:
+        sp, _ = mred.resample_interp(dev(img), sx, sy, 0, fill=-5.0)
+        ws, _ = mred.resample(dev(img), sx, sy, fill=-5.0, ws=False)
+        assert np.array_equal(host(sp), host(ws))
+
+
 # ------------------------------------------------------------------ error behaviour
 def test_error_codes():
     g = GEOMS["small"]
@@ -736,6 +797,8 @@ def test_error_codes():
     st = torch.zeros((3, 8, 8), dtype=torch.float32, device="cuda")
     with pytest.raises(mred.MredError, match="invalid argument"):
         mred.coadd(st, None, mode=7)
+    with pytest.raises(mred.MredError, match="invalid argument"):                               # minmax is a co-add mode only
+        mred.build_masters(g, raw, raw, 60.0, raw, 5.0, mode=mred.MINMAX)
     with pytest.raises(mred.MredError, match="invalid argument"):
         mred.estimate_shifts(st, 5, 2)
     with pytest.raises(mred.MredError, match="invalid argument"):
