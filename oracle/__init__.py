@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mred_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-MEDIAN, MEAN, SIGCLIP, MINMAX = 0, 1, 2, 3
+MEDIAN, MEAN, SIGCLIP, MINMAX, MEDCLIP = 0, 1, 2, 3, 4
 SPLINE, BILINEAR, NEAREST = 0, 1, 2
 PARABOLA, GAUSSIAN = 0, 1
 

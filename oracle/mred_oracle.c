@@ -39,7 +39,7 @@ typedef struct {
     int32_t x0, y0, w, h;  /* image rectangle kept by the overscan cutout (L63)               */
 } orc_geom;
 
-enum { ORC_MEDIAN = 0, ORC_MEAN = 1, ORC_SIGCLIP = 2, ORC_MINMAX = 3 };
+enum { ORC_MEDIAN = 0, ORC_MEAN = 1, ORC_SIGCLIP = 2, ORC_MINMAX = 3, ORC_MEDCLIP = 4 };
 
 /* ------------------------------------------------------------------------------------------
  * O1  overscan ("pedestal") level: per-frame mean of the overscan pixels,
@@ -96,11 +96,24 @@ static double combine_column(const double *v, int m, int mode, double ksigma, in
         alive[imin] = 0; alive[imax] = 0;
         n = m - 2;
     }
-    if (mode == ORC_SIGCLIP) {
+    if (mode == ORC_SIGCLIP || mode == ORC_MEDCLIP) {
         for (int it = 0; it < max_iter && n > 0; ++it) {
             double mu = 0.0, var = 0.0;
+            if (mode == ORC_MEDCLIP) {
+                /* NEXT-2 variant (reading Q29): the pass is centred on the MEDIAN of the survivors and sigma is their
+                 * r.m.s. about it; a single outlier among N values then sits sqrt(N) sigma out, so k = 3 clips from N = 10 */
+                double s[256]; int c = 0;
+                for (int i = 0; i < m; ++i) {
+                    if (!alive[i]) continue;
+                    double x = v[i]; int j = c - 1;
+                    while (j >= 0 && s[j] > x) { s[j + 1] = s[j]; --j; }
+                    s[j + 1] = x; ++c;
+                }
+                mu = (c & 1) ? s[c / 2] : 0.5 * (s[c / 2 - 1] + s[c / 2]);
+            } else {
             for (int i = 0; i < m; ++i) if (alive[i]) mu += v[i];
             mu /= n;
+            }
             for (int i = 0; i < m; ++i) if (alive[i]) var += (v[i] - mu) * (v[i] - mu);
             double thr = ksigma * sqrt(var / n);
             int rejected = 0;

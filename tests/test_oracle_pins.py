@@ -647,3 +647,34 @@ def test_p16_bilinear_and_nearest_resampling():
     for interp in (oracle.BILINEAR, oracle.NEAREST):
         r = oracle.resample(img[None], [3.0], [-2.0], fill=0.0, interp=interp)
         assert np.array_equal(r.out[0][0:h - 2, 3:], img[2:, :w - 3])
+
+
+def test_p17_median_centred_clip():
+    """MEDCLIP (reading Q29): N-1 values a and one value b: the median is a, the r.m.s. about it |b - a| / sqrt(N), so b
+    sits sqrt(N) sigma out and k = 3 rejects it from N = 10 on (the mean-centred clip of O6 needs N >= 11, P9), and keeps
+    it at N = 9 (sqrt(9) = 3: the tie is kept by <=); identical values are all kept; brute force against numpy."""
+    for n, rejected in ((8, False), (9, False), (10, True), (11, True), (60, True)):
+        col = np.full(n, 100.0); col[n // 2] = 160.0
+        r = oracle.combine_column(col, oracle.MEDCLIP, 3.0, 3)
+        assert r.count == (n - 1 if rejected else n), (n, r.count)
+        assert r.value == (100.0 if rejected else col.mean())
+        assert bool(r.keep[n // 2]) == (not rejected)
+    r = oracle.combine_column(np.full(7, 5.5), oracle.MEDCLIP, 3.0, 3)
+    assert r.count == 7 and r.value == 5.5
+    rng = np.random.default_rng(17)
+    for _ in range(200):
+        n = int(rng.integers(3, 40))
+        col = rng.normal(1000, 30, size=n)
+        col[rng.random(n) < 0.1] += rng.uniform(200, 5000)
+        alive = np.ones(n, bool)
+        for _it in range(3):
+            med = np.median(col[alive])
+            sig = np.sqrt(np.mean((col[alive] - med) ** 2))
+            keep = alive & (np.abs(col - med) <= 3.0 * sig)
+            if keep.sum() == alive.sum():
+                break
+            alive = keep
+            if not alive.any():
+                break
+        r = oracle.combine_column(col, oracle.MEDCLIP, 3.0, 3)
+        assert np.array_equal(r.keep, alive) and abs(r.value - (col[alive].mean() if alive.any() else 0.0)) < 1e-9
