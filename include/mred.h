@@ -48,7 +48,8 @@ typedef struct {
     int32_t x0, y0, w, h; /* image rectangle kept by the overscan cutout               */
 } mred_geom;
 
-typedef enum { MRED_MEDIAN = 0, MRED_MEAN = 1, MRED_SIGCLIP = 2, MRED_MINMAX = 3 /* mred_coadd only */ } mred_combine;
+typedef enum { MRED_MEDIAN = 0, MRED_MEAN = 1, MRED_SIGCLIP = 2,
+               MRED_MINMAX = 3, MRED_MEDCLIP = 4 /* 3, 4: mred_coadd and mred_reduce* only */ } mred_combine;
 typedef enum { MRED_PEAK_PARABOLA = 0, MRED_PEAK_GAUSSIAN = 1 } mred_peak;
 typedef enum { MRED_INTERP_SPLINE = 0, MRED_INTERP_BILINEAR = 1, MRED_INTERP_NEAREST = 2 } mred_interp;
 
@@ -171,7 +172,8 @@ int mred_resample_interp(const float *in, int n, int w, int h, const double *sx,
  * rejmask: uint32 [ceil(n/32)][h][w], bit k%32 of word k/32 set iff frame k was NOT used
  * (nullable).  No covering frame -> value 0, count 0.  mode MRED_MINMAX (Q26; mred_coadd and
  * mred_reduce* only): the mean without one minimum and one maximum (first occurrences in frame order; fewer than 3 values:
- * the plain mean).
+ * the plain mean).  mode MRED_MEDCLIP (NEXT-2, Q29): the k-sigma clip centred on the MEDIAN of the survivors, sigma = their
+ * r.m.s. about it (clips from N = 10 at k = 3, where the mean-centred clip cannot); result = mean of the survivors.
  */
 int mred_coadd(const float *stack, int n, int w, int h, const int32_t *footprint, const mred_comb_opts *opts,
                float *out, uint16_t *count, uint32_t *rejmask, void *stream);

@@ -14,7 +14,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmred.so")
 
-MEDIAN, MEAN, SIGCLIP, MINMAX = 0, 1, 2, 3
+MEDIAN, MEAN, SIGCLIP, MINMAX, MEDCLIP = 0, 1, 2, 3, 4
 PEAK_PARABOLA, PEAK_GAUSSIAN = 0, 1
 INTERP_SPLINE, INTERP_BILINEAR, INTERP_NEAREST = 0, 1, 2
 CALL_BUILD_MASTERS, CALL_CALIBRATE, CALL_ESTIMATE_SHIFTS, CALL_RESAMPLE, CALL_COADD, CALL_REDUCE, CALL_FILL_BAD = range(7)

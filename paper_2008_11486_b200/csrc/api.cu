@@ -25,9 +25,9 @@ int sm_count()
 static bool opts_ok(const mred_comb_opts* o, bool allow_minmax = false)
 {
     if (!o) return false;
-    if (o->mode != MRED_MEDIAN && o->mode != MRED_MEAN && o->mode != MRED_SIGCLIP && !(allow_minmax && o->mode == MRED_MINMAX))
+    if (o->mode != MRED_MEDIAN && o->mode != MRED_MEAN && o->mode != MRED_SIGCLIP && !(allow_minmax && (o->mode == MRED_MINMAX || o->mode == MRED_MEDCLIP)))
         return false;
-    if (o->mode == MRED_SIGCLIP && (!(o->ksigma >= 0.f) || o->max_iter < 0)) return false;
+    if ((o->mode == MRED_SIGCLIP || o->mode == MRED_MEDCLIP) && (!(o->ksigma >= 0.f) || o->max_iter < 0)) return false;
     return true;
 }
 

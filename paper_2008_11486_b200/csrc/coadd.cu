@@ -163,6 +163,40 @@ __global__ void __launch_bounds__(128) k_coadd_any(const float* __restrict__ sta
                 if (rank == ib) b = v[i];
             }
             value = 0.5f * a + 0.5f * b;
+        } else if (MODE == MRED_MEDCLIP) {
+            // NEXT-2 variant (Q29): each pass is centred on the median of the survivors (selection by rank
+            // counting), sigma = their r.m.s. about it; result = mean of the survivors.  A functional variant, not tuned.
+            for (int it = 0; it < max_iter && cnt > 0; ++it) {
+                const int ia = (cnt - 1) >> 1, ib = cnt >> 1;
+                float a = 0.f, b = 0.f;
+                for (int i = 0; i < n; ++i) {
+                    if (!used[i]) continue;
+                    int rank = 0;
+                    for (int j = 0; j < n; ++j)
+                        if (used[j] && (v[j] < v[i] || (v[j] == v[i] && j < i))) ++rank;
+                    if (rank == ia) a = v[i];
+                    if (rank == ib) b = v[i];
+                }
+                const float med = 0.5f * a + 0.5f * b;
+                float S = 0.f;
+                for (int k = 0; k < n; ++k) if (used[k]) S = fmaf(v[k] - med, v[k] - med, S);
+                const float thr = fmaf(ksigma, sqrtf(S / (float)cnt), 1e-10f * fabsf(med));
+                int ncnt = 0;
+                for (int k = 0; k < n; ++k) {
+                    if (!used[k]) continue;
+                    if (fabsf(v[k] - med) <= thr) ++ncnt; else used[k] = 0;
+                }
+                if (ncnt == cnt) break;
+                cnt = ncnt;
+            }
+            if (cnt > 0) {
+                float sum = 0.f;
+                for (int k = 0; k < n; ++k) if (used[k]) sum += v[k];
+                const float c = sum / (float)cnt;
+                float r1 = 0.f;
+                for (int k = 0; k < n; ++k) if (used[k]) r1 += v[k] - c;
+                value = c + r1 / (float)cnt;
+            }
         } else if (MODE == MRED_MINMAX) {
             // one minimum and one maximum (first occurrences) left out, mean of the rest; fewer than 3 values: plain mean
             float sum = 0.f, mn = CUDART_INF_F, mx = -CUDART_INF_F;
@@ -248,7 +282,7 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
     const int4* fpd = reinterpret_cast<const int4*>(fp_dev);
     const float ks = o.ksigma;
     const int mi = o.max_iter;
-    if (o.mode != MRED_MEDIAN && np % 4 == 0 && np >= (size_t)cs::TPS) {
+    if (o.mode != MRED_MEDIAN && o.mode != MRED_MEDCLIP && np % 4 == 0 && np >= (size_t)cs::TPS) {
         // mean / sigma-clipped mean: streaming pass + compacted clip pass on bulk-copy-staged tiles (coadd_stream.cuh);
         // planes whose size is not a multiple of 4 pixels (tiles not 16-byte aligned) keep the register kernels below
         static PerDeviceOnce once;
@@ -265,6 +299,11 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
         if (!tma::encode_f32_map(&tm, stack, 2, dims, strides, box)) { set_cuda_error(cudaErrorInvalidValue); return MRED_ECUDA; }
         k_coadd_stream<<<dim3((unsigned)((np + cs::TP - 1) / cs::TP)), cs::TP, (size_t)n * cs::TPS * 4, st>>>(
             tm, n, w, h, fpd, use_fp, local, o.mode, ks, mi, out, count, rejmask);
+        MRED_LAUNCH_CHECK();
+        return MRED_OK;
+    }
+    if (o.mode == MRED_MEDCLIP) {      // functional variant: the any-N kernel
+        k_coadd_any<MRED_MEDCLIP><<<dim3((unsigned)((np + 127) / 128)), 128, 0, st>>>(stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
         MRED_LAUNCH_CHECK();
         return MRED_OK;
     }

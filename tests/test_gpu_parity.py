@@ -738,6 +738,27 @@ def test_coadd_minmax_parity(n, aligned):
     assert np.array_equal(host(c2), r2.count) and np.array_equal(host(m2), r2.rejmask) and np.array_equal(host(o2), r2.out)
 
 
+@pytest.mark.parametrize("n", [3, 10, 11, 33, 64])
+def test_coadd_medclip_parity(n):
+    """MRED_MEDCLIP (median-centred clip) against the oracle: count and mask bit-exact away from threshold ties (margin
+    map), value at the stated bar; at N = 10 it rejects the planted hits that the mean-centred clip of O6 must keep."""
+    st, fp = _stack(n, 40, 66, 400 + n, hits=0.02)
+    ref = oracle.coadd(st, fp, mode=oracle.MEDCLIP)
+    out, cnt, mask = mred.coadd(dev(st), fp, mode=mred.MEDCLIP, want_mask=True)
+    safe = ref.margin >= 1e-3 + 1e-5 * 100.0
+    yy, xx = np.mgrid[0:st.shape[1], 0:st.shape[2]]
+    m = sum(((xx >= f[0]) & (xx <= f[1]) & (yy >= f[2]) & (yy <= f[3])).astype(int) for f in fp)
+    safe |= m <= 1                                                # a lone value is its own median: margin 0, no decision
+    assert (~safe).mean() < 5e-3
+    assert np.array_equal(host(cnt)[safe], ref.count[safe])
+    for wd in range(ref.rejmask.shape[0]):
+        assert np.array_equal(host(mask)[wd][safe], ref.rejmask[wd][safe])
+    assert_close(host(out)[safe], ref.out[safe], "coadd medclip n %d" % n)
+    if n == 10:
+        plain = oracle.coadd(st, fp, mode=oracle.SIGCLIP)
+        assert (ref.count < plain.count).mean() > 0.05            # it clips where Samuelson's bound forbids the mean-centred clip
+
+
 def test_estimate_shifts_gaussian_peak():
     """MRED_PEAK_GAUSSIAN against the oracle on a star field (within 1e-3 px, integer part identical) and on Gaussian
     profiles, where it recovers the injected sub-pixel shift itself."""
