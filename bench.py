@@ -215,17 +215,17 @@ ALL_STAGES = ["build_masters"] + STAGES
 
 def kernels_per_group(mred, g, n, masked):
     """Kernels this repo launches per group and step (memset nodes not counted): mred_build_masters = k_master_sums,
-    k_masters_bd, k_masters_f, k_mf_scale; mred_reduce = k_frame_sums, [k_mask_counts], k_calibrate_prof, k_finalize,
-    k_correlate, the resample kernel(s) (one tiled kernel, or x kernel + y kernel on small planes), the co-add kernel."""
+    k_masters_bd, k_masters_f, k_mf_scale; mred_reduce = k_frame_sums, [k_mask_counts], k_calibrate_prof, k_estimate,
+    the resample kernel(s) (one tiled kernel, or x kernel + y kernel on small planes), the co-add kernel."""
     resample = 2 if mred.workspace_bytes(mred.CALL_RESAMPLE, g, n) else 1
-    return 4 + 4 + (1 if masked else 0) + resample + 1
+    return 4 + 3 + (1 if masked else 0) + resample + 1
 
 
 def stage_kernels(mred, g, n, mode):
     tiled = g.w % 4 == 0 and g.w >= 256 and g.h >= 64
     return {"build_masters": "k_masters_bd + k_masters_f (+ k_master_sums, k_mf_scale)",
             "calibrate": "k_calibrate_prof (+ k_frame_sums)",
-            "estimate_shifts": "k_finalize, k_correlate (profile sums come from k_calibrate_prof)",
+            "estimate_shifts": "k_estimate (profile sums come from k_calibrate_prof)",
             "resample": "k_resample_tile (TMA-staged, x + y fused)" if tiled else "k_resample<1> + k_ypass4 (x pass, y pass)",
             "coadd": "k_coadd_stream (bulk-copy staged)" if mode != 0 and (g.w * g.h) % 4 == 0 else "k_coadd<N,MODE>"}
 

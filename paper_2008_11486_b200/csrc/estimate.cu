@@ -4,10 +4,9 @@
 //
 //   k_profiles : one streaming pass over the frames (the only HBM traffic, N*4wh B): fixed-point (int64) column
 //                partial sums per 32-row band and complete row sums, valid-pixel counts.
-//   k_finalize : per (frame, axis): mean from the integer sums, median by a bitonic sort (registers + shuffles inside
-//                a warp, shared memory across warps), subtract.
-//   k_correlate: per (frame, axis): C(l) = sum_j a[j] b[j+l], l in [-R, R]; argmax with ties to the
-//                smaller |l| then smaller l; 3-point parabola.
+//   k_estimate : per (frame, axis): mean from the integer sums, median by a bitonic sort (registers + shuffles inside
+//                a warp, shared memory across warps), subtract; C(l) = sum_j a[j] b[j+l], l in [-R, R] against the
+//                reference profile; argmax with ties to the smaller |l| then smaller l; 3-point parabola.
 // No float atomics: every sum has a fixed order, so the integer result is reproducible.
 #include "common.cuh"
 
@@ -254,62 +253,61 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
     __syncthreads();
 }
 
-// grid (n, 2), block 1024: median-subtracted mean profile of (frame, axis) -> e.prof
-__global__ void __launch_bounds__(1024) k_finalize(int w, int h, int has_bad, EstimateWs e)
+// ---------------------------------------------------------------------------------------------
+// k_estimate: profile finishing AND lag search of one (frame, axis) per block (round 1 had two kernels, k_finalize and
+// k_correlate: 28-36 us of dependent latency per stack).  grid (n, 2), block 1024.  Block x = 0 takes the REFERENCE frame:
+// it writes its median-subtracted profile to e.prof and raises a flag (the zeroed ticket of (ref, axis)); every other block
+// finishes its own profile (the bitonic sort is the long part, and runs in parallel with the reference's), then waits for
+// the flag -- a block only ever waits for the block with x = 0 of its own axis, which precedes it in dispatch order, the
+// decoupled look-back pattern -- stages the reference profile in the shared memory the sort no longer needs, and takes
+//   C(l) = sum_j a[j] b[j+l], l in [-R, R]   (float64, one lag per warp at a time), the argmax with ties to the smaller |l|
+// then the smaller l, and the 3-point (log-)parabola.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_estimate(int w, int h, int n, int ref, int R, int peak, int has_bad, EstimateWs e,
+                                                   int32_t* __restrict__ ishift, double* __restrict__ shift)
 {
-    extern __shared__ double s_dyn[];     // profile[P], sort keys[P]
+    extern __shared__ double s_dyn[];     // own profile b[P], then sort keys[P] / reference profile a[len]
     __shared__ int s_m;
-    const int k = blockIdx.x, axis = blockIdx.y;
+    __shared__ double sC[2 * MRED_MAX_LAG + 1];
+    const int axis = blockIdx.y;
+    const int bx = blockIdx.x;
+    const int k = bx == 0 ? ref : (bx <= ref ? bx - 1 : bx);
     const int len = axis == 0 ? w : h;
     int P = 1;
     while (P < len) P <<= 1;
-    double* a = s_dyn;
+    double* b = s_dyn;
     unsigned long long* keys = reinterpret_cast<unsigned long long*>(s_dyn + P);
-    block_profile(e, w, h, k, axis, len, P, has_bad, a, keys, &s_m);
-    double* out = e.prof + ((size_t)k * 2 + axis) * e.plen;
-    for (int i = threadIdx.x; i < len; i += blockDim.x) out[i] = a[i];
-}
-
-// grid (n, 2, CORR_Z), block 256: C(l) = sum_j a[j] b[j+l] (float64: the one place it is kept, ~65 k DFMA per
-// profile pair, spread over CORR_Z blocks because vector FP64 is scarce per SM), both profiles staged in shared
-// memory, lags dealt round-robin to the warps of the CORR_Z blocks; the last block of a (frame, axis) to finish
-// takes the argmax (ties: smaller |l|, then smaller l) and the 3-point parabola.
-constexpr int CORR_Z = 8;
-__global__ void __launch_bounds__(256) k_correlate(int w, int h, int n, int ref, int R, int peak, EstimateWs e,
-                                                   int32_t* __restrict__ ishift, double* __restrict__ shift)
-{
-    extern __shared__ double s_dyn[];     // a[len], b[len]
-    __shared__ int s_last;
-    const int k = blockIdx.x, axis = blockIdx.y;
+    block_profile(e, w, h, k, axis, len, P, has_bad, b, keys, &s_m);
+    double* gref = e.prof + ((size_t)ref * 2 + axis) * e.plen;
+    unsigned int* flag = e.ticket + 2 * ref + axis;
     if (k == ref) {
-        if (threadIdx.x == 0 && blockIdx.z == 0) { ishift[2 * k + axis] = 0; shift[2 * k + axis] = 0.0; }
+        for (int i = threadIdx.x; i < len; i += blockDim.x) gref[i] = b[i];
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            atomicExch(flag, 1u);
+            ishift[2 * k + axis] = 0;
+            shift[2 * k + axis] = 0.0;
+        }
         return;
     }
-    const int len = axis == 0 ? w : h;
-    double* a = s_dyn;
-    double* b = s_dyn + len;
-    const double* ga = e.prof + ((size_t)ref * 2 + axis) * e.plen;
-    const double* gb = e.prof + ((size_t)k * 2 + axis) * e.plen;
-    for (int i = threadIdx.x; i < len; i += blockDim.x) { a[i] = ga[i]; b[i] = gb[i]; }
+    if (threadIdx.x == 0) {
+        while (atomicAdd(flag, 0u) == 0u) __nanosleep(200);
+        __threadfence();
+    }
+    __syncthreads();
+    double* a = reinterpret_cast<double*>(keys);          // the sort is done: its scratch holds the reference profile
+    for (int i = threadIdx.x; i < len; i += blockDim.x) a[i] = __ldcg(gref + i);
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double* C = e.corr + ((size_t)k * 2 + axis) * (2 * MRED_MAX_LAG + 1);
-    for (int q = (int)blockIdx.z + CORR_Z * warp; q <= 2 * R; q += CORR_Z * 8) {
+    for (int q = warp; q <= 2 * R; q += 32) {
         const int l = q - R;
         const int j0 = max(0, -l), j1 = min(len, len - l);
         double s = 0.0;
         for (int j = j0 + lane; j < j1; j += 32) s = fma(a[j], b[j + l], s);
         s = warp_sum(s);
-        if (lane == 0) C[q] = s;
+        if (lane == 0) sC[q] = s;
     }
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(e.ticket + 2 * k + axis, 1u) == CORR_Z - 1);
-    __syncthreads();
-    if (!s_last) return;
-    double* sC = s_dyn;                      // the profiles are no longer needed: reuse their space (2R+1 <= 2 len)
-    __syncthreads();
-    for (int q = threadIdx.x; q <= 2 * R; q += blockDim.x) sC[q] = __ldcg(C + q);
     __syncthreads();
     if (threadIdx.x != 0) return;
     int best = 0;
@@ -356,13 +354,11 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     static PerDeviceOnce once;
     int dev;
     if (once.pending(dev)) {
-        MRED_CUDA_TRY(cudaFuncSetAttribute(k_finalize, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
-        MRED_CUDA_TRY(cudaFuncSetAttribute(k_correlate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
+        MRED_CUDA_TRY(cudaFuncSetAttribute(k_estimate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
         once.mark(dev);
     }
-    k_finalize<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, bad ? ((flags & EST_SHARED_COUNTS) ? 2 : 1) : 0, e);
-    MRED_LAUNCH_CHECK();
-    k_correlate<<<dim3(n, 2, CORR_Z), 256, 2 * (size_t)(w > h ? w : h) * sizeof(double), st>>>(w, h, n, ref, max_lag, peak, e, ishift, shift);
+    k_estimate<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, n, ref, max_lag, peak,
+                                                                        bad ? ((flags & EST_SHARED_COUNTS) ? 2 : 1) : 0, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
