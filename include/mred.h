@@ -41,6 +41,7 @@ extern "C" {
 #define MRED_MAX_STACK 255
 #define MRED_MAX_LAG 256
 #define MRED_MAX_PROFILE 4096 /* longest row / column mred_estimate_shifts and mred_reduce* accept */
+#define MRED_STATIC_SCRATCH_BYTES (4u << 20) /* the built-in scratch of mred_estimate_shifts_static, per device */
 
 typedef struct {
     int32_t W, H;         /* raw frame size, x fastest (1074 x 1024 incl. overscan)   */
@@ -64,7 +65,8 @@ typedef enum {
     MRED_EINVAL = -1,     /* null pointer, bad shape/geometry/count/option                          */
     MRED_EALIGN = -2,     /* a device pointer is not 16-byte aligned                                */
     MRED_EWORKSPACE = -3, /* ws is null or smaller than mred_workspace_bytes()                      */
-    MRED_ECUDA = -4       /* a CUDA runtime call failed; see mred_last_cuda_error()                 */
+    MRED_ECUDA = -4,      /* a CUDA runtime call failed; see mred_last_cuda_error()                 */
+    MRED_ELIMIT = -5      /* the problem needs more scratch than a no-allocation entry point holds  */
 } mred_status;
 
 typedef enum {
@@ -136,6 +138,22 @@ int mred_estimate_shifts(const float *frames, int n, int w, int h, int ref_index
 int mred_estimate_shifts_peak(const float *frames, int n, int w, int h, int ref_index, int max_lag,
                               const uint8_t *badmask, int peak, int32_t *ishift, double *shift, void *ws,
                               size_t ws_bytes, void *stream);
+
+/*
+ * mred_estimate_shifts_peak for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no workspace argument.  The scratch is a static device array of
+ * MRED_STATIC_SCRATCH_BYTES (4 MiB) inside the library, held by every device that loads the library until the process
+ * exits; the call itself calls no cudaMalloc / cudaFree and no allocating library routine.  Results are those of
+ * mred_estimate_shifts_peak, bit for bit (same kernels, O4).
+ * Limit: mred_workspace_bytes(MRED_CALL_ESTIMATE_SHIFTS, {w, h}, n) <= MRED_STATIC_SCRATCH_BYTES, else MRED_ELIMIT and
+ * nothing is enqueued (64 frames of 1024 x 1024 need 3.1 MiB; 100 frames of 4096 x 4096 do not fit).
+ * Every call on a device shares the one array, which keeps the previous call's contents: the call clears what has to
+ * start at zero (on `stream`, before its kernels), and calls that may OVERLAP on the GPU (different streams, or graph
+ * branches) race on it -- serialise them.  The first call on a device looks up the array's device address
+ * (cudaGetSymbolAddress, kept per device); make that first call outside a stream capture.
+ */
+int mred_estimate_shifts_static(const float *frames, int n, int w, int h, int ref_index, int max_lag,
+                                const uint8_t *badmask, int peak, int32_t *ishift, double *shift, void *stream);
 
 /*
  * Sub-pixel shift by bicubic (tensor-product natural cubic) spline interpolation (PAPER.md L63,

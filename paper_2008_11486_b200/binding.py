@@ -23,6 +23,7 @@ MAX_STACK = 255
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
            "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
            "mred_reduce_workspace_views", "mred_fill_bad", "mred_reduce_filled", "mred_estimate_shifts_peak", "mred_resample_interp",
+           "mred_estimate_shifts_static",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -186,6 +187,25 @@ def estimate_shifts(frames, ref_index=0, max_lag=32, badmask=None, ws=None, stre
                                          C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream(stream))
     _check(rc, "mred_estimate_shifts")
     return ish, sh
+
+
+STATIC_SCRATCH_BYTES = 4 << 20
+
+
+def estimate_shifts_static(frames, ishift, shift, ref_index=0, max_lag=32, badmask=None, stream=None, peak=0):
+    """include/mred.h: mred_estimate_shifts_static -- no workspace and no allocation, here or in the library: the caller
+    passes the outputs (ishift int32 [n][2], shift float64 [n][2], device).  MredError (MRED_ELIMIT) when the stack needs
+    more than STATIC_SCRATCH_BYTES of scratch."""
+    n, h, w = frames.shape
+    _shape(badmask, (h, w), "badmask")
+    _shape(ishift, (n, 2), "ishift")
+    _shape(shift, (n, 2), "shift")
+    rc = lib().mred_estimate_shifts_static(_dev(frames, torch.float32, "frames"), C.c_int(n), C.c_int(w), C.c_int(h),
+                                           C.c_int(ref_index), C.c_int(max_lag), _dev(badmask, torch.uint8, "badmask"),
+                                           C.c_int(peak), _dev(ishift, torch.int32, "ishift"),
+                                           _dev(shift, torch.float64, "shift"), _stream(stream))
+    _check(rc, "mred_estimate_shifts_static")
+    return ishift, shift
 
 
 def resample(frames, sx, sy, fill=0.0, out=None, ws=None, stream=None):

@@ -123,6 +123,7 @@ const char* mred_strerror(int status)
         case MRED_EALIGN: return "device pointer not 16-byte aligned";
         case MRED_EWORKSPACE: return "workspace missing or too small";
         case MRED_ECUDA: return "CUDA runtime error (see mred_last_cuda_error)";
+        case MRED_ELIMIT: return "problem exceeds the static scratch of the no-allocation entry point (MRED_STATIC_SCRATCH_BYTES)";
         default: return "unknown status";
     }
 }
@@ -212,6 +213,20 @@ int mred_estimate_shifts(const float* frames, int n, int w, int h, int ref_index
 {
     return mred_estimate_shifts_peak(frames, n, w, h, ref_index, max_lag, badmask, MRED_PEAK_PARABOLA, ishift, shift, ws,
                                      ws_bytes, stream);
+}
+
+int mred_estimate_shifts_static(const float* frames, int n, int w, int h, int ref_index, int max_lag,
+                                const uint8_t* badmask, int peak, int32_t* ishift, double* shift, void* stream)
+{
+    if (!frames || !ishift || !shift || n < 1 || n > MRED_MAX_STACK || w < 1 || h < 1) return MRED_EINVAL;
+    if (w > MRED_MAX_PROFILE || h > MRED_MAX_PROFILE) return MRED_EINVAL;
+    if (ref_index < 0 || ref_index >= n || max_lag < 0 || max_lag > MRED_MAX_LAG || max_lag >= w || max_lag >= h)
+        return MRED_EINVAL;
+    if (peak != MRED_PEAK_PARABOLA && peak != MRED_PEAK_GAUSSIAN) return MRED_EINVAL;
+    if (!aligned16(frames) || !aligned16(ishift) || !aligned16(shift) || (badmask && !aligned16(badmask)))
+        return MRED_EALIGN;
+    return launch_estimate_static(frames, n, w, h, ref_index, max_lag, badmask, ishift, shift, peak,
+                                  static_cast<cudaStream_t>(stream));
 }
 
 int mred_resample(const float* in, int n, int w, int h, const double* sx, const double* sy, float fill,

@@ -134,6 +134,9 @@ int launch_mask_counts(const uint8_t* bad, int w, int h, int n, void* ws, cudaSt
 int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
                     int32_t* ishift, double* shift, void* ws, int flags, int peak /* 0 parabola, 1 log-parabola */, cudaStream_t st);
 size_t estimate_ws_bytes(int w, int h, int n);
+// launch_estimate on the library's own static device scratch (estimate.cu); MRED_ELIMIT when it is too small
+int launch_estimate_static(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
+                           int32_t* ishift, double* shift, int peak, cudaStream_t st);
 // the accumulators inside an estimate workspace: what has to be zero before the sums start, and where they are
 void estimate_accumulators(void* ws, int w, int h, int n, void** zero, size_t* zero_bytes, long long** colsum, long long** rowsum);
 int launch_resample(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host,

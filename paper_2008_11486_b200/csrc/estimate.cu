@@ -363,4 +363,30 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
     return MRED_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// mred_estimate_shifts_static: the scratch of the estimate kernels in a file-scope device array instead of a caller's
+// workspace, for callers that cannot allocate (include/mred.h).  Every device that loads the library holds the
+// MRED_STATIC_SCRATCH_BYTES of it until the process exits.  In HOST code the array's name is only a handle of the host
+// side, not a device address, so the address the kernels get is looked up with cudaGetSymbolAddress, once per device
+// with that device current, and kept.  All calls share the array: launch_estimate clears the accumulators and the
+// flags at its top (cudaMemsetAsync on the stream), and calls that overlap on the GPU would race on it.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_estimate_scratch[MRED_STATIC_SCRATCH_BYTES];
+
+int launch_estimate_static(const float* frames, int n, int w, int h, int ref, int max_lag, const uint8_t* bad,
+                           int32_t* ishift, double* shift, int peak, cudaStream_t st)
+{
+    if (estimate_ws_bytes(w, h, n) > (size_t)MRED_STATIC_SCRATCH_BYTES) return MRED_ELIMIT;
+    static std::atomic<void*> addr[64];
+    int dev = -1;
+    MRED_CUDA_TRY(cudaGetDevice(&dev));
+    void* p = (dev >= 0 && dev < 64) ? addr[dev].load(std::memory_order_acquire) : nullptr;
+    if (!p) {
+        MRED_CUDA_TRY(cudaGetSymbolAddress(&p, g_estimate_scratch));
+        if (!p) { set_cuda_error(cudaErrorInvalidSymbol); return MRED_ECUDA; }
+        if (dev >= 0 && dev < 64) addr[dev].store(p, std::memory_order_release);
+    }
+    return launch_estimate(frames, n, w, h, ref, max_lag, bad, ishift, shift, p, 0, peak, st);
+}
+
 }  // namespace mred
