@@ -88,6 +88,7 @@ __device__ __forceinline__ Axis make_axis(int n, double s)
 #include "resample_warp.cuh"
 #include "resample_ypass.cuh"
 #include "resample_tile.cuh"
+#include "resample_pipe.cuh"
 #include "resample_lin.cuh"
 
 namespace mred {
@@ -118,9 +119,9 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
     if (!dshift_dev)
         for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
     int4* fpd = reinterpret_cast<int4*>(fp_dev);
-    // planes with 16-byte-aligned rows, at least 256 x 64: the CTA-tiled TMA kernel (resample_tile.cuh); smaller or
-    // unaligned planes: the warp kernels below
-    if (rt::tile_route(w, h)) return rt::launch_resample_tile(in, n, w, h, hs, dshift_dev, fill, out, fpd, st);
+    // planes with 16-byte-aligned rows, at least 256 x 64: the CTA-tiled, TMA-staged pipeline (resample_pipe.cuh, with the
+    // row / column code of resample_tile.cuh); smaller or unaligned planes: the warp kernels below
+    if (rt::tile_route(w, h)) return rp::launch_resample_pipe(in, n, w, h, hs, dshift_dev, fill, out, fpd, st);
     const int vec = (w % 4 == 0) ? 1 : 0;
     const size_t smem = (size_t)NRING * RB * WARPCOLS * sizeof(float);
     static PerDeviceOnce once;

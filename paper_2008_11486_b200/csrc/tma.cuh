@@ -21,6 +21,10 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t by
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity)
 {
     uint32_t ok;
@@ -44,6 +48,27 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
             if ((threadIdx.x & 31) == 0) printf("mred: TMA wait timed out (block %d, warp %d, parity %u)\n", (int)blockIdx.x, (int)(threadIdx.x >> 5), parity);
             __trap();
         }
+}
+// The same wait for barriers whose phase may take a while (another warp role is behind): the try_wait carries a
+// suspend-time hint, so the warp is parked by the hardware instead of re-issuing the poll every few cycles.
+__device__ __forceinline__ void mbar_wait_parked(uint64_t* bar, uint32_t parity)
+{
+    uint32_t spins = 0;
+    while (true) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity), "r"(2000u)
+            : "memory");
+        if (ok) return;
+        if (++spins > (1u << 22)) {
+            if ((threadIdx.x & 31) == 0) printf("mred: barrier wait timed out (block %d, warp %d, parity %u)\n", (int)blockIdx.x, (int)(threadIdx.x >> 5), parity);
+            __trap();
+        }
+    }
 }
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int x, int y, int z, uint64_t* bar)
 {
