@@ -226,7 +226,7 @@ def stage_kernels(mred, g, n, mode):
     return {"build_masters": "k_masters_bd + k_masters_f (+ k_master_sums, k_mf_scale)",
             "calibrate": "k_calibrate_prof (+ k_frame_sums)",
             "estimate_shifts": "k_estimate (profile sums come from k_calibrate_prof)",
-            "resample": "k_resample_tile (TMA-staged, x + y fused)" if tiled else "k_resample<1> + k_ypass4 (x pass, y pass)",
+            "resample": "k_resample_pipe (TMA-staged warp-specialised pipeline, x + y fused)" if tiled else "k_resample<1> + k_ypass4 (x pass, y pass)",
             "coadd": "k_coadd_stream (bulk-copy staged)" if mode != 0 and (g.w * g.h) % 4 == 0 else "k_coadd<N,MODE>"}
 
 

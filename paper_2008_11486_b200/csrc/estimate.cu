@@ -20,7 +20,7 @@ constexpr int PROF_MAXLEN = MRED_MAX_PROFILE;  // longest profile the finalize k
 struct EstimateWs {
     long long* colpart;  // [n][w]   fixed-point column sums (value * FIX), accumulated with integer atomics by the bands
     int* colcnt;      // [n][w]   valid rows per column (contiguous after colpart: zeroed together; used with a mask only)
-    unsigned int* ticket;  // [n][2] block counters of k_correlate (contiguous after colcnt: zeroed by the same memset)
+    unsigned int* ticket;  // [n][2] flags of k_estimate (contiguous after colcnt: zeroed by the same memset)
     long long* rowsum;   // [n][h]
     int* rowcnt;      // [n][h]
     double* prof;     // [n][2][plen]  median-subtracted profiles (x then y)
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256) k_profiles(const float* __restrict__ fram
 }
 
 // Valid-pixel counts per column and per row of the bad-pixel mask, into the count arrays of frame 0 (the mask is the
-// same for every frame of a stack, so the chained path counts once and k_finalize reads frame 0's counts for all frames).
+// same for every frame of a stack, so the chained path counts once and k_estimate reads frame 0's counts for all frames).
 // grid (nbands), block 256; the arrays must be zero on entry.
 __global__ void __launch_bounds__(256) k_mask_counts(const uint8_t* __restrict__ bad, int w, int h, EstimateWs e)
 {

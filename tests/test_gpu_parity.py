@@ -501,7 +501,7 @@ def test_config3_group_full_size_chained():
 
 def test_config4_full_size_chained_with_badmask():
     """BASELINE.json config 4 through mred_reduce with its real hot-column bad-pixel mask: 64 frames, cosmic rays,
-    saturated stars; the masked fused calibrate kernel, k_mask_counts, the shared counts in k_finalize, the 64-frame
+    saturated stars; the masked fused calibrate kernel, k_mask_counts, the shared counts in k_estimate, the 64-frame
     co-add with a 2-word rejection mask.  Registered planes compared on a sample of frames."""
     grp = synth.make_group(4)
     assert grp.badmask is not None and grp.badmask.any()
