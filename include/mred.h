@@ -41,6 +41,7 @@ extern "C" {
 #define MRED_MAX_STACK 255
 #define MRED_MAX_LAG 256
 #define MRED_MAX_PROFILE 4096 /* longest row / column mred_estimate_shifts and mred_reduce* accept */
+#define MRED_HOST_CHUNKS 4 /* pieces mred_reduce_host_overlapped copies the raw stack in */
 #define MRED_STATIC_SCRATCH_BYTES (4u << 20) /* the built-in scratch of mred_estimate_shifts_static, per device */
 
 typedef struct {
@@ -243,6 +244,23 @@ int mred_reduce_host(const mred_geom *geom, const uint16_t *raw_host, int n, flo
                      const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
                      float fill, const mred_comb_opts *opts, float *out_host, uint16_t *count_host,
                      double *shift_host, void *ws, size_t ws_bytes, void *stream);
+
+/*
+ * mred_reduce_host with the host->device copy OVERLAPPED with the calibration inside the call (PAPER.md
+ * Table 6: transfers and I/O are 64 % of the paper's run): the raw stack is copied in up to MRED_HOST_CHUNKS pieces of
+ * whole frames on `copy_stream`, and the overscan levels, the calibration and the profile sums of each piece are enqueued
+ * on `stream` behind an event of its copy, so piece c is calibrated while piece c + 1 is still on the bus; estimate_shifts,
+ * resample and coadd follow on `stream` as in mred_reduce.  Results are bit-identical to mred_reduce_host.
+ * The library creates nothing: copy_stream (a second cudaStream_t, != stream) and events (HOST array of MRED_HOST_CHUNKS + 1
+ * cudaEvent_t, timing may be disabled) come from the caller and may be reused by the next call.  On return everything is
+ * enqueued; `stream` has been made to wait for every copy, so synchronising `stream` also covers copy_stream's work.
+ * raw_host should be pinned memory (pageable memory makes the copies synchronous).  Same workspace as mred_reduce_host.
+ */
+int mred_reduce_host_overlapped(const mred_geom *geom, const uint16_t *raw_host, int n, float dark_scale, const float *MB,
+                                const float *MD, const float *MF, int ref_index, int max_lag, const uint8_t *badmask,
+                                float fill, const mred_comb_opts *opts, float *out_host, uint16_t *count_host,
+                                double *shift_host, void *ws, size_t ws_bytes, void *stream, void *copy_stream,
+                                void *const *events);
 
 /*
  * Where mred_reduce / mred_reduce_staged leave their two intermediate stacks inside `ws` (byte offsets from ws):

@@ -23,7 +23,7 @@ MAX_STACK = 255
 EXPORTS = ["mred_build_masters", "mred_calibrate", "mred_estimate_shifts", "mred_resample", "mred_coadd",
            "mred_reduce", "mred_reduce_staged", "mred_reduce_host", "mred_workspace_bytes", "mred_reduce_host_workspace_bytes",
            "mred_reduce_workspace_views", "mred_fill_bad", "mred_reduce_filled", "mred_estimate_shifts_peak", "mred_resample_interp",
-           "mred_estimate_shifts_static",
+           "mred_estimate_shifts_static", "mred_reduce_host_overlapped",
            "mred_strerror", "mred_last_cuda_error", "mred_version"]
 
 
@@ -375,4 +375,36 @@ def reduce_host(plan: ReducePlan, raw_host, dark_scale, MB, MD, MF, ref_index=0,
                                 C.c_void_p(plan.shift.data_ptr()), C.c_void_p(plan.ws.data_ptr()),
                                 C.c_size_t(plan.ws.numel()), _stream(stream))
     _check(rc, "mred_reduce_host")
+    return plan
+
+
+HOST_CHUNKS = 4
+
+
+def reduce_host_overlapped(plan: ReducePlan, raw_host, dark_scale, MB, MD, MF, copy_stream, events, ref_index=0, max_lag=32,
+                           badmask=None, fill=0.0, mode=SIGCLIP, ksigma=3.0, max_iter=3, stream=None):
+    """include/mred.h: mred_reduce_host_overlapped -- mred_reduce_host with the host->device copy in HOST_CHUNKS pieces on
+    `copy_stream` (a torch.cuda.Stream other than `stream`), each piece calibrated while the next is on the bus.
+    events: HOST_CHUNKS + 1 torch.cuda.Event objects, reusable from call to call.  Results as reduce_host."""
+    if raw_host.is_cuda or raw_host.dtype != torch.uint16 or not raw_host.is_contiguous():
+        raise MredError("raw_host must be a contiguous CPU uint16 tensor")
+    if not plan.host:
+        raise MredError("reduce_host_overlapped needs a ReducePlan(host=True)")
+    if len(events) != HOST_CHUNKS + 1:
+        raise MredError("events must hold HOST_CHUNKS + 1 torch.cuda.Event objects")
+    _reduce_shapes(plan, raw_host, MB, MD, MF, badmask)
+    o = _opts(mode, ksigma, max_iter)
+    for e in events:
+        if e.cuda_event == 0:          # torch creates the CUDA event lazily, on first record
+            e.record(copy_stream)
+    ev = (C.c_void_p * (HOST_CHUNKS + 1))(*[C.c_void_p(e.cuda_event) for e in events])
+    rc = lib().mred_reduce_host_overlapped(C.byref(plan.g), C.c_void_p(raw_host.data_ptr()), C.c_int(plan.n),
+                                           C.c_float(dark_scale), _dev(MB, torch.float32, "MB"), _dev(MD, torch.float32, "MD"),
+                                           _dev(MF, torch.float32, "MF"), C.c_int(ref_index), C.c_int(max_lag),
+                                           _dev(badmask, torch.uint8, "badmask"), C.c_float(fill), C.byref(o),
+                                           C.c_void_p(plan.out.data_ptr()),
+                                           C.c_void_p(plan.count.data_ptr() if plan.count is not None else None),
+                                           C.c_void_p(plan.shift.data_ptr()), C.c_void_p(plan.ws.data_ptr()),
+                                           C.c_size_t(plan.ws.numel()), _stream(stream), C.c_void_p(copy_stream.cuda_stream), ev)
+    _check(rc, "mred_reduce_host_overlapped")
     return plan

@@ -290,6 +290,56 @@ int mred_reduce_workspace_views(const mred_geom* geom, int n, size_t* calibrated
     return MRED_OK;
 }
 
+// The science path in two parts, so that mred_reduce_host_overlapped can run the first one chunk by chunk while the rest
+// of the stack is still on its way to the device.
+//   reduce_calibrate: frames [c0, c0 + nc) of the raw stack: overscan levels, calibration, and the marginal profile sums
+//   of O4 (left in the accumulators of the estimate workspace).  The call for c0 == 0 also clears those accumulators and
+//   takes the valid-pixel counts of the bad-pixel mask, so it has to be enqueued first.
+//   reduce_finish: estimate_shifts from the sums, (fill,) resample, coadd.
+static int reduce_calibrate(const Geom& g, const uint16_t* raw, int n, int c0, int nc, float dark_scale, const float* MB,
+                            const float* MD, const float* MF, const uint8_t* badmask, const ReduceWs& r, cudaStream_t st)
+{
+    // The level kernel also clears the accumulators of estimate_shifts (no memset node between the stages); the
+    // calibrate kernel sums the marginal profiles itself (leaving out masked pixels), so estimate_shifts starts at
+    // its finalize step and the calibrated stack is not re-read.
+    void* zero;
+    size_t zero_bytes;
+    long long *colsum, *rowsum;
+    estimate_accumulators(r.est, g.w, g.h, n, &zero, &zero_bytes, &colsum, &rowsum);
+    const int nos = frame_sums_parts(g);
+    const uint16_t* rawc = raw + (size_t)c0 * g.W * g.H;
+    unsigned long long* osc = r.os + (size_t)c0 * nos;
+    int rc;
+    if ((rc = launch_frame_sums(rawc, g, nc, osc, c0 == 0 ? zero : nullptr, c0 == 0 ? zero_bytes : 0, st))) return rc;
+    if (c0 == 0 && badmask)      // the mask is the same for every frame: its valid-pixel counts are taken once
+        if ((rc = launch_mask_counts(badmask, g.w, g.h, n, r.est, st))) return rc;
+    return launch_calibrate_prof(rawc, g, nc, dark_scale, MB, MD, MF, r.cal + (size_t)c0 * g.w * g.h, osc, badmask,
+                                 colsum + (size_t)c0 * g.w, rowsum + (size_t)c0 * g.h, st);
+}
+
+#define MRED_STAGE_EVENT(i) \
+    do { if (events && events[i]) MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[i]), st)); } while (0)
+
+static int reduce_finish(const Geom& g, int n, int ref_index, int max_lag, const uint8_t* badmask, float fill,
+                         const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
+                         int32_t* footprint_out, const ReduceWs& r, cudaStream_t st, void* const* events, bool fill_bad)
+{
+    int rc;
+    const int est_flags = EST_ZEROED | EST_HAVE_SUMS | (badmask ? EST_SHARED_COUNTS : 0);
+    double* shift = shift_out ? shift_out : r.shift;
+    int32_t* fp = footprint_out ? footprint_out : r.fp;
+    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, est_flags, MRED_PEAK_PARABOLA, st))) return rc;
+    MRED_STAGE_EVENT(2);
+    // bad-pixel fill (O7) between the calibrated stack and its resampling: a hot pixel would otherwise ring through the
+    // spline prefilter; the profile sums above were taken without the masked pixels, so the shifts do not depend on it
+    if (fill_bad && (rc = launch_fill_bad(r.cal, n, g.w, g.h, badmask, r.fill, st))) return rc;
+    if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, r.rs, r.rs_bytes, st))) return rc;
+    MRED_STAGE_EVENT(3);
+    if ((rc = launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st))) return rc;
+    MRED_STAGE_EVENT(4);
+    return MRED_OK;
+}
+
 static int reduce_impl(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
                        const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
                        const mred_comb_opts* opts, float* out, uint16_t* count, uint32_t* rejmask, double* shift_out,
@@ -303,38 +353,13 @@ static int reduce_impl(const mred_geom* geom, const uint16_t* raw, int n, float 
     if (!ws || !aligned16(ws) || ws_bytes < carve_reduce(nullptr, g, n).bytes) return MRED_EWORKSPACE;
     const ReduceWs r = carve_reduce(ws, g, n);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-#define MRED_STAGE_EVENT(i) \
-    do { if (events && events[i]) MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[i]), st)); } while (0)
     MRED_STAGE_EVENT(0);
-    // The level kernel also clears the accumulators of estimate_shifts (no memset node between the stages); the
-    // calibrate kernel sums the marginal profiles itself (leaving out masked pixels), so estimate_shifts starts at
-    // its finalize kernel and the calibrated stack is not re-read.
-    void* zero;
-    size_t zero_bytes;
-    long long *colsum, *rowsum;
-    estimate_accumulators(r.est, g.w, g.h, n, &zero, &zero_bytes, &colsum, &rowsum);
-    if ((rc = launch_frame_sums(raw, g, n, r.os, zero, zero_bytes, st))) return rc;
-    int est_flags = EST_ZEROED | EST_HAVE_SUMS;
-    if (badmask) {      // the mask is the same for every frame: its valid-pixel counts are taken once
-        if ((rc = launch_mask_counts(badmask, g.w, g.h, n, r.est, st))) return rc;
-        est_flags |= EST_SHARED_COUNTS;
-    }
-    if ((rc = launch_calibrate_prof(raw, g, n, dark_scale, MB, MD, MF, r.cal, r.os, badmask, colsum, rowsum, st))) return rc;
+    if ((rc = reduce_calibrate(g, raw, n, 0, n, dark_scale, MB, MD, MF, badmask, r, st))) return rc;
     MRED_STAGE_EVENT(1);
-    double* shift = shift_out ? shift_out : r.shift;
-    int32_t* fp = footprint_out ? footprint_out : r.fp;
-    if ((rc = launch_estimate(r.cal, n, g.w, g.h, ref_index, max_lag, badmask, r.ishift, shift, r.est, est_flags, MRED_PEAK_PARABOLA, st))) return rc;
-    MRED_STAGE_EVENT(2);
-    // bad-pixel fill (O7) between the calibrated stack and its resampling: a hot pixel would otherwise ring through the
-    // spline prefilter; the profile sums above were taken without the masked pixels, so the shifts do not depend on it
-    if (fill_bad && (rc = launch_fill_bad(r.cal, n, g.w, g.h, badmask, r.fill, st))) return rc;
-    if ((rc = launch_resample(r.cal, n, g.w, g.h, nullptr, nullptr, shift, fill, r.reg, fp, r.rs, r.rs_bytes, st))) return rc;
-    MRED_STAGE_EVENT(3);
-    if ((rc = launch_coadd(r.reg, n, g.w, g.h, nullptr, fp, *opts, out, count, rejmask, st))) return rc;
-    MRED_STAGE_EVENT(4);
-#undef MRED_STAGE_EVENT
-    return MRED_OK;
+    return reduce_finish(g, n, ref_index, max_lag, badmask, fill, opts, out, count, rejmask, shift_out, footprint_out, r, st,
+                         events, fill_bad);
 }
+#undef MRED_STAGE_EVENT
 
 int mred_reduce_staged(const mred_geom* geom, const uint16_t* raw, int n, float dark_scale, const float* MB,
                        const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask, float fill,
@@ -383,6 +408,48 @@ int mred_reduce_host(const mred_geom* geom, const uint16_t* raw_host, int n, flo
                      count_host ? hw.count : nullptr, nullptr, r.shift, nullptr, hw.reduce,
                      carve_reduce(nullptr, g, n).bytes, stream);
     if (rc) return rc;
+    MRED_CUDA_TRY(cudaMemcpyAsync(out_host, hw.out, 4 * np, cudaMemcpyDeviceToHost, st));
+    if (count_host) MRED_CUDA_TRY(cudaMemcpyAsync(count_host, hw.count, 2 * np, cudaMemcpyDeviceToHost, st));
+    if (shift_host) MRED_CUDA_TRY(cudaMemcpyAsync(shift_host, r.shift, 16 * (size_t)n, cudaMemcpyDeviceToHost, st));
+    return MRED_OK;
+}
+
+int mred_reduce_host_overlapped(const mred_geom* geom, const uint16_t* raw_host, int n, float dark_scale, const float* MB,
+                                const float* MD, const float* MF, int ref_index, int max_lag, const uint8_t* badmask,
+                                float fill, const mred_comb_opts* opts, float* out_host, uint16_t* count_host,
+                                double* shift_host, void* ws, size_t ws_bytes, void* stream, void* copy_stream,
+                                void* const* events)
+{
+    if (!raw_host || !out_host || !events || !copy_stream || copy_stream == stream) return MRED_EINVAL;
+    for (int i = 0; i <= MRED_HOST_CHUNKS; ++i)
+        if (!events[i]) return MRED_EINVAL;
+    int rc = reduce_args_ok(geom, n, MB, MD, MF, ref_index, max_lag, badmask, opts, nullptr, nullptr, nullptr, nullptr);
+    if (rc) return rc;
+    const Geom g = to_geom(geom);
+    if (!ws || !aligned16(ws) || ws_bytes < carve_host(nullptr, g, n).bytes) return MRED_EWORKSPACE;
+    const HostWs hw = carve_host(ws, g, n);
+    const ReduceWs r = carve_reduce(hw.reduce, g, n);
+    cudaStream_t st = static_cast<cudaStream_t>(stream), cs = static_cast<cudaStream_t>(copy_stream);
+    const size_t np = (size_t)g.w * g.h, fb = 2 * (size_t)g.W * g.H;
+    // chunks of whole calibrate blocks (4 frames), at most MRED_HOST_CHUNKS of them
+    int per = (n + MRED_HOST_CHUNKS - 1) / MRED_HOST_CHUNKS;
+    per = (per + 3) / 4 * 4;
+    // the copies may not start before what `stream` still does with the workspace has finished
+    MRED_CUDA_TRY(cudaEventRecord(static_cast<cudaEvent_t>(events[0]), st));
+    MRED_CUDA_TRY(cudaStreamWaitEvent(cs, static_cast<cudaEvent_t>(events[0]), 0));
+    int ci = 0;
+    for (int c0 = 0; c0 < n; c0 += per, ++ci) {
+        const int nc = n - c0 < per ? n - c0 : per;
+        MRED_CUDA_TRY(cudaMemcpyAsync(reinterpret_cast<char*>(hw.raw) + (size_t)c0 * fb, reinterpret_cast<const char*>(raw_host) + (size_t)c0 * fb,
+                                      (size_t)nc * fb, cudaMemcpyHostToDevice, cs));
+        cudaEvent_t ev = static_cast<cudaEvent_t>(events[1 + ci]);
+        MRED_CUDA_TRY(cudaEventRecord(ev, cs));
+        MRED_CUDA_TRY(cudaStreamWaitEvent(st, ev, 0));
+        if ((rc = reduce_calibrate(g, hw.raw, n, c0, nc, dark_scale, MB, MD, MF, badmask, r, st))) return rc;
+    }
+    if ((rc = reduce_finish(g, n, ref_index, max_lag, badmask, fill, opts, hw.out, count_host ? hw.count : nullptr, nullptr,
+                            r.shift, nullptr, r, st, nullptr, false)))
+        return rc;
     MRED_CUDA_TRY(cudaMemcpyAsync(out_host, hw.out, 4 * np, cudaMemcpyDeviceToHost, st));
     if (count_host) MRED_CUDA_TRY(cudaMemcpyAsync(count_host, hw.count, 2 * np, cudaMemcpyDeviceToHost, st));
     if (shift_host) MRED_CUDA_TRY(cudaMemcpyAsync(shift_host, r.shift, 16 * (size_t)n, cudaMemcpyDeviceToHost, st));

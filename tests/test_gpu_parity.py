@@ -654,6 +654,37 @@ def test_reduce_host_matches_reduce():
             mred.reduce_host(hplan, raw_host, 1.0, MB, MD, MF, n + 3, 12, badmask=bad, mode=mode)
 
 
+def test_reduce_host_overlapped_matches_reduce():
+    """mred_reduce_host_overlapped (the raw stack copied in pieces on a copy stream, each piece calibrated
+    while the next is on the bus) must return bit for bit what mred_reduce returns: the profile sums are integer
+    atomics, so the piecewise calibration cannot change them.  Frame counts that are not a multiple of the piece size,
+    fewer frames than pieces, a bad-pixel mask, and two calls in a row on the same plan, streams and events."""
+    cases = [synth.make_group(1, geom=synth.GEOM_SMALL, stars=30, S=6.0),                                   # 5 frames
+             synth.make_group(4, geom=synth.GEOM_SMALL, stars=30, S=6.0, n_sci=23, n_master=4),             # mask, 23 frames
+             synth.make_group(2, geom=synth.GEOM_SMALL, stars=30, S=6.0, n_sci=2, n_master=3),              # 2 frames: one piece
+             synth.make_group(1)]                                                                            # full size
+    cs = torch.cuda.Stream()
+    evs = [torch.cuda.Event() for _ in range(mred.HOST_CHUNKS + 1)]
+    for grp in cases:
+        g, n = grp.geom, grp.sci.shape[0]
+        mode = grp.coadd
+        MB, MD, MF = mred.build_masters(g, dev(grp.bias), dev(grp.dark), grp.t_dark, dev(grp.flat), grp.t_flat)
+        bad = dev(grp.badmask) if grp.badmask is not None else None
+        plan = mred.ReducePlan(g, n)
+        mred.reduce(plan, dev(grp.sci), 1.0, MB, MD, MF, 0, 12, badmask=bad, mode=mode)
+        hplan = mred.ReducePlan(g, n, host=True)
+        raw_host = torch.from_numpy(np.ascontiguousarray(grp.sci)).pin_memory()
+        for rep in range(2):
+            hplan.out.zero_()
+            mred.reduce_host_overlapped(hplan, raw_host, 1.0, MB, MD, MF, cs, evs, 0, 12, badmask=bad, mode=mode)
+            torch.cuda.synchronize()
+            assert np.array_equal(hplan.out.numpy(), host(plan.out))
+            assert np.array_equal(hplan.count.numpy(), host(plan.count))
+            assert np.array_equal(hplan.shift.numpy(), host(plan.shift))
+        with pytest.raises(mred.MredError, match="invalid argument"):       # the copy stream must differ from the stream
+            mred.reduce_host_overlapped(hplan, raw_host, 1.0, MB, MD, MF, torch.cuda.current_stream(), evs, 0, 12, badmask=bad, mode=mode)
+
+
 def test_estimate_shifts_tie_rule():
     """O4(iv) on exact ties (the frames of the oracle pin test_p7_argmax_tie_rule): C(-5) == C(+2) -> +2,
     C(-3) == C(+3) -> -3, C(-2) == C(+5) -> -2, C(-4) == C(+3) -> +3, sub-pixel part exactly 0; through the stand-alone
