@@ -11,8 +11,9 @@
  * Conventions (all calls):
  *  - Every array pointer is DEVICE memory owned by the caller unless the comment says "host".
  *    The library never allocates, frees or retains a pointer and keeps no global mutable state
- *    (apart from the last CUDA error code, see mred_last_cuda_error); calls on different
- *    streams are independent.
+ *    (apart from the last CUDA error code, see mred_last_cuda_error, and the static device scratch of
+ *    mred_estimate_shifts_static, which only that call touches); calls on different streams are
+ *    independent.
  *  - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
  *    stream) and the call returns WITHOUT synchronising, except mred_reduce_host which
  *    returns after its device->host copies are enqueued (also not synchronised).

@@ -161,10 +161,17 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__
     const size_t np = (size_t)w * h;
     const size_t p0 = (size_t)blockIdx.x * TP;
     const int tp = (int)min((size_t)TP, np - p0);           // pixels of this tile (a multiple of 4)
+    // stage the tile: ONE tensor copy, a box of TPS pixels x n frames out of the [n][w*h] stack, issued before anything else
+    // so that the classification of the frames below runs under the copy.  (One 512-byte bulk copy per frame, 60 per tile,
+    // held the whole kernel at 3.5 TB/s: the copy engine takes a copy every ~40 cycles per SM whatever its size.)  The box
+    // is 4 pixels wider than the tile, so the rows land with the 132-float pitch that keeps pass B free of bank conflicts;
+    // pixels beyond the plane arrive as zeros and are never looked at.
     if (tid == 0) {
         s_nall = 0; s_nnone = 0; s_nd = 0; s_nnf = 0;
         tma::mbar_init(&s_bar, 1);
         tma::fence_mbar_init();
+        tma::mbar_arrive_expect_tx(&s_bar, (uint32_t)n * (uint32_t)TPS * 4u);
+        tma::tma_load_2d(vals, &tmap, (int)p0, 0, &s_bar);
     }
     __syncthreads();
     // classify every frame against the tile's pixels [p0, p0 + tp)
@@ -191,14 +198,6 @@ __global__ void __launch_bounds__(cs::TP) k_coadd_stream(const __grid_constant__
         }
     }
     __syncthreads();
-    // stage the tile: ONE tensor copy, a box of TPS pixels x n frames out of the [n][w*h] stack.  (One 512-byte bulk copy
-    // per frame, 60 per tile, held the whole kernel at 3.5 TB/s: the copy engine takes a copy every ~40 cycles per SM
-    // whatever its size.)  The box is 4 pixels wider than the tile, so the rows land with the 132-float pitch that keeps
-    // pass B free of bank conflicts; pixels beyond the plane arrive as zeros and are never looked at.
-    if (tid == 0) {
-        tma::mbar_arrive_expect_tx(&s_bar, (uint32_t)n * (uint32_t)TPS * 4u);
-        tma::tma_load_2d(vals, &tmap, (int)p0, 0, &s_bar);
-    }
     const bool live = tid < tp;
     const size_t p = p0 + tid;
     float* col = vals + tid;
