@@ -452,6 +452,33 @@ def bench_config(cfg, args, steps, warmup, mred, torch, dist, devs, rank, world,
     return res
 
 
+def bench_fill(mred, torch, dev):
+    """mred_fill_bad (k_fill_plan + k_fill_apply) timed with CUDA events, 20 reps after 3 warm-ups, L2 flushed between."""
+    n, h, w = 64, 1024, 1024
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(20200826)
+    stack = torch.randn((n, h, w), device=dev, generator=gen) * 30 + 1000
+    bad = (torch.rand((h, w), device=dev, generator=gen) < 1e-4).to(torch.uint8)
+    bad[:, 100:1000:90] = 1
+    ws = torch.empty(mred.workspace_bytes(mred.CALL_FILL_BAD, (0, 0, 0, 0, 0, 0, w, h), n), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ts = []
+    for i in range(23):
+        flush.fill_(i & 1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        mred.fill_bad(stack, bad, ws=ws)
+        b.record()
+        torch.cuda.synchronize()
+        if i >= 3:
+            ts.append(a.elapsed_time(b))
+    ts.sort()
+    nbad = int(bad.sum().item())
+    return {"workload": "64 x 1024x1024 float32, %d masked pixels per frame (10 hot columns + 1e-4 isolated)" % nbad,
+            "us_per_call": round(1e3 * ts[len(ts) // 2], 2), "frames_per_s": round(n / (1e-3 * ts[len(ts) // 2]), 0),
+            "kernels": "k_fill_plan (once per mask) + k_fill_apply"}
+
+
 def load_traffic(cfg):
     """DRAM bytes per stage call (dram__bytes_read.sum + dram__bytes_write.sum of the stage's kernels) from the ncu
     --set full capture of this round's build on this config: profiles/r2_traffic.csv, written from profiles/r2_kernels.md."""
@@ -527,6 +554,13 @@ def run_ours(args):
                 extra["config %d" % c] = summary(r2)
             except Exception as exc:                     # an extra must never cost the headline
                 extra["config %d" % c] = {"error": repr(exc)[:200]}
+
+        # NEXT-1: the bad-pixel fill on a config-4-like stack (64 x 1024^2, 10 hot columns + 1e-4 isolated
+        # pixels), the paper's second-largest GPU stage (Table 6: 0.36 s per 540 frames on its hardware)
+        try:
+            extra["fill_bad"] = bench_fill(mred, torch, devs)
+        except Exception as exc:
+            extra["fill_bad"] = {"error": repr(exc)[:200]}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
