@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
     }
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
-    const float ABSENT = (MODE == MRED_MEDIAN) ? CUDART_INF_F : CUDART_NAN_F;
+    const float ABSENT = (MODE == MRED_MEDIAN || MODE == MRED_MEDCLIP) ? CUDART_INF_F : CUDART_NAN_F;
     float v[NMAX];
     uint32_t inside[NW];
 #pragma unroll
@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
 #pragma unroll
     for (int i = 0; i < NW; ++i) m += __popc(inside[i]);
     const float* src = stack + p;
-    if (MODE != MRED_MEDIAN && NMAX <= 24 && n == NMAX && m == NMAX) {
+    if (MODE != MRED_MEDIAN && MODE != MRED_MEDCLIP && NMAX <= 24 && n == NMAX && m == NMAX) {
         // short column, every frame covers this pixel (the usual case; with 32+ frames some lane of the warp
         // nearly always rejects something and the attempt would be wasted): unconditional loads, and a clip loop that only has to
         // find out that nothing is rejected (bit-identical to the general path below, which takes over otherwise)
@@ -100,6 +100,22 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
         r = combine_median<NMAX>(v, m);
 #pragma unroll
         for (int i = 0; i < (NMAX + 31) / 32; ++i) rej[i] = ~inside[i];
+    } else if (MODE == MRED_MEDCLIP) {
+        // the sort has lost which value belongs to which frame: a frame was used iff its value lies in the survivors' range,
+        // so for the mask the column is read once more (out of L2; only when a mask is asked for)
+        float vlo, vhi;
+        r = combine_medclip<NMAX>(v, m, ksigma, max_iter, vlo, vhi);
+#pragma unroll
+        for (int i = 0; i < (NMAX + 31) / 32; ++i) rej[i] = ~inside[i];
+        if (rejmask && r.count < m) {
+            const float* s2 = stack + p;
+#pragma unroll
+            for (int k = 0; k < NMAX; ++k) {
+                const bool ok = (inside[k >> 5] >> (k & 31)) & 1u;
+                if (ok) { const float t = __ldg(s2); if (t < vlo || t > vhi) rej[k >> 5] |= 1u << (k & 31); }
+                s2 += np;
+            }
+        }
     } else {
         r = combine_mean_clip<NMAX>(v, m, MODE == MRED_SIGCLIP, ksigma, max_iter);
 #pragma unroll
@@ -266,6 +282,8 @@ static void launch_mode(int mode, dim3 grid, cudaStream_t st, const float* stack
         k_coadd<NMAX, MRED_MEDIAN><<<grid, 256, 0, st>>>(stack, n, w, h, fp_dev, use_fp, hfp, ks, mi, out, count, rejmask);
     else if (mode == MRED_MEAN)
         k_coadd<NMAX, MRED_MEAN><<<grid, 256, 0, st>>>(stack, n, w, h, fp_dev, use_fp, hfp, ks, mi, out, count, rejmask);
+    else if (mode == MRED_MEDCLIP)
+        k_coadd<NMAX, MRED_MEDCLIP><<<grid, 256, 0, st>>>(stack, n, w, h, fp_dev, use_fp, hfp, ks, mi, out, count, rejmask);
     else
         k_coadd<NMAX, MRED_SIGCLIP><<<grid, 256, 0, st>>>(stack, n, w, h, fp_dev, use_fp, hfp, ks, mi, out, count, rejmask);
 }
@@ -302,7 +320,7 @@ int launch_coadd(const float* stack, int n, int w, int h, const int32_t* fp_host
         MRED_LAUNCH_CHECK();
         return MRED_OK;
     }
-    if (o.mode == MRED_MEDCLIP) {      // functional variant: the any-N kernel
+    if (o.mode == MRED_MEDCLIP && n > 128) {      // above the largest register capacity: the any-N kernel
         k_coadd_any<MRED_MEDCLIP><<<dim3((unsigned)((np + 127) / 128)), 128, 0, st>>>(stack, n, w, h, fpd, use_fp, local, ks, mi, out, count, rejmask);
         MRED_LAUNCH_CHECK();
         return MRED_OK;

@@ -78,6 +78,71 @@ __device__ __forceinline__ Combined combine_median(float (&v)[NMAX], int m)
     return r;
 }
 
+// Median-centred clip (Q29): each pass is centred on the median of the survivors, sigma =
+// their r.m.s. about it, keep |v - med| <= k sigma; the result is the mean of the survivors.  The column is SORTED once
+// (absent entries hold +INF and sort to the end); a pass can only reject from the two ends of the sorted survivors, so
+// they stay a contiguous range [lo, hi], whose median is the middle slot(s).  On exit [vlo, vhi] is the value range of
+// the survivors (empty: vlo > vhi): frame k was used iff its value lies inside, which is how the caller builds the mask.
+template <int NMAX>
+__device__ __forceinline__ Combined combine_medclip(float (&v)[NMAX], int m, float ksigma, int max_iter, float& vlo, float& vhi)
+{
+    Combined r;
+    r.count = m;
+    r.value = 0.f;
+    vlo = CUDART_INF_F;
+    vhi = -CUDART_INF_F;
+    if (m <= 0) return r;
+    sort_network<NMAX>(v);
+    int lo = 0, hi = m - 1;
+    for (int it = 0; it < max_iter && lo <= hi; ++it) {
+        const int cnt = hi - lo + 1;
+        const int ia = lo + ((cnt - 1) >> 1), ib = lo + (cnt >> 1);
+        float a = 0.f, b = 0.f;
+#pragma unroll
+        for (int i = 0; i < NMAX; ++i) {
+            a = (i == ia) ? v[i] : a;
+            b = (i == ib) ? v[i] : b;
+        }
+        const float med = 0.5f * a + 0.5f * b;
+        float S = 0.f;
+#pragma unroll
+        for (int i = 0; i < NMAX; ++i) {
+            const float d = v[i] - med;
+            S = (i >= lo && i <= hi) ? fmaf(d, d, S) : S;
+        }
+        const float thr = fmaf(ksigma, sqrtf(S / (float)cnt), 1e-10f * fabsf(med));
+        int nlo = 0, nhi = 0;
+#pragma unroll
+        for (int i = 0; i < NMAX; ++i) {
+            const float d = v[i] - med;
+            const bool in = i >= lo && i <= hi;
+            nlo += (in && d < -thr) ? 1 : 0;
+            nhi += (in && d > thr) ? 1 : 0;
+        }
+        if (nlo + nhi == 0) break;
+        lo += nlo;
+        hi -= nhi;
+    }
+    const int cnt = hi - lo + 1;
+    r.count = cnt > 0 ? cnt : 0;
+    if (cnt > 0) {
+        float sum = 0.f;
+#pragma unroll
+        for (int i = 0; i < NMAX; ++i) {
+            const bool in = i >= lo && i <= hi;
+            sum += in ? v[i] : 0.f;
+            vlo = (i == lo) ? v[i] : vlo;
+            vhi = (i == hi) ? v[i] : vhi;
+        }
+        const float c = sum / (float)cnt;
+        float r1 = 0.f;
+#pragma unroll
+        for (int i = 0; i < NMAX; ++i) r1 += (i >= lo && i <= hi) ? v[i] - c : 0.f;
+        r.value = c + r1 / (float)cnt;
+    }
+    return r;
+}
+
 // Fast path of the mean / sigma-clipped mean for a column whose NMAX entries are all present: the same float
 // operations in the same order as combine_mean_clip (so the same bits), without the absent-entry bookkeeping,
 // and v[] is left untouched.  Returns false when the first clip pass would reject something: the caller then runs

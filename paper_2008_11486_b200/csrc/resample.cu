@@ -167,10 +167,13 @@ int launch_resample(const float* in, int n, int w, int h, const double* sx_host,
 int launch_resample_lin(const float* in, int n, int w, int h, const double* sx_host, const double* sy_host, int interp,
                         float fill, float* out, cudaStream_t st)
 {
-    HostShifts hs;
-    for (int k = 0; k < n; ++k) { hs.s[k][0] = sx_host[k]; hs.s[k][1] = sy_host[k]; }
-    const size_t np = (size_t)w * h;
-    k_resample_lin<<<dim3((unsigned)((np + 255) / 256), (unsigned)n), 256, 0, st>>>(in, w, h, hs, interp, fill, out);
+    rl::LinAxes axes;
+    for (int k = 0; k < n; ++k) {
+        axes.a[k][0] = rl::make_lin_axis(w, sx_host[k], interp);
+        axes.a[k][1] = rl::make_lin_axis(h, sy_host[k], interp);
+    }
+    if ((h + RL_ROWS - 1) / RL_ROWS > 65535) return MRED_EINVAL;
+    k_resample_lin<<<dim3((unsigned)((w + 255) / 256), (unsigned)((h + RL_ROWS - 1) / RL_ROWS), (unsigned)n), 256, 0, st>>>(in, w, h, axes, fill, out);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
