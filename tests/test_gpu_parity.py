@@ -769,7 +769,7 @@ def test_coadd_minmax_parity(n, aligned):
     assert np.array_equal(host(c2), r2.count) and np.array_equal(host(m2), r2.rejmask) and np.array_equal(host(o2), r2.out)
 
 
-@pytest.mark.parametrize("n", [3, 10, 11, 33, 64])
+@pytest.mark.parametrize("n", [3, 10, 11, 33, 64, 130])
 def test_coadd_medclip_parity(n):
     """MRED_MEDCLIP (median-centred clip) against the oracle: count and mask bit-exact away from threshold ties (margin
     map), value at the stated bar; at N = 10 it rejects the planted hits that the mean-centred clip of O6 must keep."""
