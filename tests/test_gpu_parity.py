@@ -805,6 +805,57 @@ def test_estimate_shifts_gaussian_peak():
     assert np.max(np.abs(host(sh) - np.array([[0, 0], [2.3, -1.4], [-1.45, 1.2]]))) < 2e-4
 
 
+def test_resample_random_shapes_and_shifts():
+    """Seeded sweep of the tiled TMA route (k_resample_pipe): 50 random stacks (64..520 rows, 256..1316 columns, 1..6 frames:
+    every size moves the run boundaries, the chunk grid and the number of pipelines) with shifts of every kind on either axis
+    -- fractional, integer (copies), tiny, larger than the frame, half-pixel -- against the oracle at the stated bar
+    (star fields without saturated spikes, Q18b); footprints and copies bit-exact."""
+    rng = np.random.default_rng(12345)
+    worst = 0.0
+    for case in range(50):
+        h = int(rng.integers(64, 520))
+        w = max(256, int(rng.integers(64, 330)) * 4)
+        if case % 7 == 0:
+            h = int(rng.choice([64, 65, 79, 80, 81, 95, 96, 97, 128, 255, 256, 257]))
+        if case % 11 == 0:
+            w = int(rng.choice([256, 260, 416, 420, 464, 624, 628, 1024, 1040]))
+        n = int(rng.integers(1, 7))
+        img = rng.normal(1000.0, 30.0, size=(n, h, w)).astype(np.float32)
+        yy, xx = np.mgrid[0:h, 0:w]
+        for k in range(n):
+            for _ in range(5):
+                x, y, a = rng.uniform(0, w), rng.uniform(0, h), np.exp(rng.uniform(np.log(200), np.log(20000)))
+                img[k] += (a * np.exp(-0.5 * ((xx - x) ** 2 + (yy - y) ** 2) / 1.274 ** 2)).astype(np.float32)
+        kind = rng.integers(0, 5, size=(n, 2))
+        sx, sy = np.zeros(n), np.zeros(n)
+        for k in range(n):
+            for ax, arr, size in ((0, sx, w), (1, sy, h)):
+                t = kind[k, ax]
+                if t == 0:
+                    arr[k] = rng.uniform(-30, 30)
+                elif t == 1:
+                    arr[k] = float(rng.integers(-20, 21))                 # integer: a copy along this axis
+                elif t == 2:
+                    arr[k] = rng.uniform(-size * 1.2, size * 1.2)          # may leave the frame entirely
+                elif t == 3:
+                    arr[k] = rng.uniform(-1, 1) * 1e-6
+                else:
+                    arr[k] = rng.integers(-5, 6) + rng.choice([0.5, 0.25, 0.999, 0.001])
+        ref = oracle.resample(img, sx, sy)
+        out, fp = mred.resample(dev(img), sx, sy)
+        got = host(out)
+        assert np.array_equal(fp, ref.footprint), (case, h, w, n)
+        d = np.abs(got.astype(np.float64) - ref.out)
+        tol = 1e-3 + 1e-5 * np.abs(ref.out)
+        r = float((d / tol).max())
+        worst = max(worst, r)
+        assert r <= 1.0, (case, h, w, n, r, sx.tolist(), sy.tolist())
+        for k in range(n):
+            if sx[k] == np.floor(sx[k]) and sy[k] == np.floor(sy[k]):
+                assert np.array_equal(got[k], ref.out[k].astype(np.float32)), (case, k)
+    print("resample random sweep: worst ratio to the stated bar %.3f" % worst)
+
+
 @pytest.mark.parametrize("interp", [1, 2])
 @pytest.mark.parametrize("shape", [(136, 192), (71, 183), (300, 420)])
 def test_resample_interp_parity(shape, interp):
