@@ -14,14 +14,18 @@
 // With NR = 4 ring slots the x warps run up to two chunks ahead of the y warps, so neither role waits for the other's
 // slowest warp.  Every arrival is one lane per warp after __syncwarp(); every wait is a warp-wide try_wait with a
 // suspend-time hint (a plain polling loop took 40 % of the issue slots).
-// A CTA holds NPIPE = 2 independent pipelines (1024 threads, each pipeline its own run of segments, stages, ring and
-// barriers) with their warps INTERLEAVED (pipeline = warp & 1).  As two CTAs of 512 threads the pipeline that was launched
-// second on an SM ran 25 % slower than the first (the warp scheduler favours the older CTA) and then finished alone, at
-// half occupancy; interleaved, both finish together.
+// A CTA is one pipeline of 512 threads, two per SM (NPIPE = 1).  Measured against it: NPIPE = 2, two pipelines in one CTA of
+// 1024 threads with their warps interleaved (pipeline = warp & 1).  As two CTAs the pipeline launched second on an SM runs
+// 25 % slower than the first (the warp scheduler favours the older CTA) and finishes alone; interleaved in one CTA both
+// finish together, which is worth 1 % when the kernel has the GPU to itself (config 3: 136.7 against 138.1 us, config 5
+// 2.93 against 2.98 ms).  But a CTA that needs a whole SM's registers can only start on an SM that is completely free: in
+// the 6-stream step of bench.py, where other groups' kernels hold parts of every SM, the 512-thread CTAs find room
+// earlier and their neighbours fill the issue slots this latency-bound kernel leaves: 1.89 -> 1.84 ms per step (+ 2.7 %
+// frames/s).  The step is what the library is for, so NPIPE = 1 it is.
 // The two configured detector widths (1024, 4096) get an instantiation with the output pitch compiled in: the 16 stores
 // of a sweep then take immediate offsets from one base register instead of a pointer chain whose every update waited for
 // the store before it to have read its address (config 3: 144 -> 138 us).
-// Shared memory per pipeline: 3 x 16 KB stages + 4 x 13 KB ring = 100 KB; registers <= 64: 32 warps per SM.
+// Shared memory per pipeline: 3 x 16 KB stages + 4 x 13 KB ring = 100 KB; registers <= 64: two pipelines = 32 warps per SM.
 #pragma once
 #include "resample_tile.cuh"
 
@@ -37,7 +41,7 @@ constexpr int YW = (TW + 31) / 32;           // y warps: one column per thread (
 constexpr int NTHR_P = (XW + YW + 1) * 32;   // + the producer warp: 512 threads
 constexpr int NS = 3;                        // TMA stages
 constexpr int NR = 4;                        // ring slots
-constexpr int NPIPE = 2;                     // independent pipelines per CTA (their warps interleaved: warp & 1)
+constexpr int NPIPE = 1;                     // pipelines per CTA (2: warps interleaved, pipeline = warp & 1; see above)
 constexpr size_t SMEM_1 = (size_t)NS * STAGE_FLOATS * 4 + (size_t)NR * T_FLOATS * 4 + 128;   // one pipeline: stages, ring, barriers
 constexpr size_t SMEM_P = SMEM_1 * NPIPE;
 
