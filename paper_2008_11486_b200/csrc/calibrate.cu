@@ -158,13 +158,17 @@ __global__ void __launch_bounds__(256) k_calibrate(const uint16_t* __restrict__ 
 // calibrate + marginal profiles in one pass (chained path; an optional bad-pixel mask keeps pixels out of the sums): the calibrated pixels are summed
 // into the row / column profiles of O4 while they are still in registers, so estimate_shifts never re-reads the
 // calibrated stack (N*4wh bytes of HBM traffic and a kernel less; SURVEY 8(d) "0 if fused into calibrate").
-// Block = 512 threads = tile of 128 columns x 16 rows (warp = one 128-pixel row segment, lane = 4 pixels) of 4
-// frames; all loads of a thread are issued up front.  Row segment sums by warp shuffle; column sums over the 16
+// Block = 256 threads = tile of 128 columns x 8 rows (warp = one 128-pixel row segment, lane = 4 pixels) of 4
+// frames; all loads of a thread are issued up front.  Row segment sums by warp shuffle; column sums over the 8
 // rows through shared memory (one barrier, then thread = (frame, column)); both are added to the global int64
 // fixed-point accumulators (value * 2^14) with integer atomics: exact and order-independent.
-// grid (ceil(n/4), ceil(w/128), ceil(h/16)).
+// Tiles of 16 rows (512 threads, half as many column atomics) measured 1-2 % slower (config 3 90.5 against 89.9 us,
+// config 5 2.08 against 2.04 ms: twice as many warps wait at the barrier for the slowest one's loads), tiles of 4 rows
+// slower again (92.3 us).
+// grid (ceil(n/4), ceil(w/128), ceil(h/8)).
 // ---------------------------------------------------------------------------------------------
-constexpr int CP_ROWS = 16, CP_COLS = 128, CP_FB = 4;     // tile and frames per block
+constexpr int CP_ROWS = 8, CP_COLS = 128, CP_FB = 4;      // tile and frames per block
+constexpr int CP_THREADS = 32 * CP_ROWS;                  // one warp per row of the tile
 
 // NKF > 0 (fast body): the tile lies inside the image, holds exactly NKF frames, rows are 16-byte aligned in the
 // output and 4-byte aligned in the raw frames: no per-thread bounds, tails or alignment tests (they were 40 % of the
@@ -183,8 +187,8 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
     // masters come out of HBM once and out of L2 for the other chunks (they exceed L2 at 4096^2)
     const int k0 = blockIdx.x * CP_FB, nk = FAST ? NKF : min(CP_FB, n - k0);
     // (the last warp takes the levels: its float64 division then delays nobody else's loads)
-    if (threadIdx.x >= 512 - CP_FB && (int)threadIdx.x - (512 - CP_FB) < nk)
-        s_level[threadIdx.x - (512 - CP_FB)] = (float)level_of(os_part, nos, k0 + (int)threadIdx.x - (512 - CP_FB), g);
+    if (threadIdx.x >= CP_THREADS - CP_FB && (int)threadIdx.x - (CP_THREADS - CP_FB) < nk)
+        s_level[threadIdx.x - (CP_THREADS - CP_FB)] = (float)level_of(os_part, nos, k0 + (int)threadIdx.x - (CP_THREADS - CP_FB), g);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x = blockIdx.y * CP_COLS + 4 * lane, y = blockIdx.z * CP_ROWS + warp;
     const bool live = FAST || (x < g.w && y < g.h);
@@ -283,8 +287,9 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
             atomicAdd(reinterpret_cast<unsigned long long*>(rowsum) + (size_t)(k0 + jf) * g.h + y, (unsigned long long)__float2ll_rn(kk * PROF_FIX));
     }
     __syncthreads();
-    {   // 512 threads = 4 frames x 128 columns: 16 rows in a fixed order
-        const int j = threadIdx.x >> 7, c = threadIdx.x & (CP_COLS - 1);
+    // thread = (frame, column): the tile's rows in a fixed order
+    for (int jc = threadIdx.x; jc < CP_FB * CP_COLS; jc += CP_THREADS) {
+        const int j = jc >> 7, c = jc & (CP_COLS - 1);
         const int cx = blockIdx.y * CP_COLS + c;
         if (FAST ? (j < NKF) : (j < nk && cx < g.w)) {
             float t = 0.f;
@@ -295,7 +300,7 @@ __device__ __forceinline__ void calibrate_prof_body(const uint16_t* __restrict__
     }
 }
 
-__global__ void __launch_bounds__(512, 3) k_calibrate_prof(const uint16_t* __restrict__ raw, Geom g, int n,
+__global__ void __launch_bounds__(CP_THREADS, 1536 / CP_THREADS) k_calibrate_prof(const uint16_t* __restrict__ raw, Geom g, int n,
                                                            float dark_scale, const float* __restrict__ MB,
                                                            const float* __restrict__ MD, const float* __restrict__ MF,
                                                            float* __restrict__ out, const unsigned long long* __restrict__ os_part,
@@ -337,7 +342,7 @@ int launch_calibrate_prof(const uint16_t* raw, const Geom& g, int n, float dark_
     dim3 grid((unsigned)((n + CP_FB - 1) / CP_FB), (unsigned)tx, (unsigned)ty);
     const int vec_ok = (g.w % 4 == 0) ? 1 : 0;
     const int pair_ok = (g.W % 2 == 0 && g.x0 % 2 == 0) ? 1 : 0;     // raw rows of the image rectangle start 4-byte aligned
-    k_calibrate_prof<<<grid, 512, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), bad, colsum, rowsum, vec_ok, pair_ok);
+    k_calibrate_prof<<<grid, CP_THREADS, 0, st>>>(raw, g, n, dark_scale, MB, MD, MF, out, os_part, frame_sums_parts(g), bad, colsum, rowsum, vec_ok, pair_ok);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
 }
