@@ -27,13 +27,19 @@ struct MastersWs {            // layout of the caller's workspace (all 16-byte a
 };
 
 constexpr int MPX = 2;        // pixels per thread in the combine kernels (one 32-bit load per frame)
+// Threads per block of the combine kernels.  Long columns (60+ registers per thread) run in blocks of 128: measured at 20
+// frames the kernels themselves gain 2 % and bench.py's 6-stream step 2.7 % (1.84 -> 1.79 ms: a block of 128 threads finds
+// room on an SM that other groups' kernels share, one of 256 has to wait for a quarter of it); short columns keep 256 (at
+// 10 frames blocks of 128 were 12-19 % SLOWER: 59 -> 66 us at 1024^2, 528 -> 628 us at 4096^2).
+constexpr int MT_MAX = 256, MT_MIN = 128;
+template <int NMAX> __host__ __device__ constexpr int masters_threads() { return NMAX >= 16 ? MT_MIN : MT_MAX; }
 
 static MastersWs carve(void* ws, const Geom& g, int nb, int nd, int nf)
 {
     MastersWs m;
     char* p = static_cast<char*>(ws);
     auto take = [&](size_t b) { char* q = p; p += align_up(b, 16); return q; };
-    const size_t nblocks = ((size_t)g.w * g.h + 255) / 256;     // upper bound for either pixels-per-thread
+    const size_t nblocks = ((size_t)g.w * g.h + MT_MIN - 1) / MT_MIN;   // upper bound for either pixels-per-thread and block size
     m.os = reinterpret_cast<unsigned long long*>(take(8 * (size_t)(nb + nd + nf)));
     m.img_f = reinterpret_cast<unsigned long long*>(take(8 * (size_t)nf));
     m.ticket = reinterpret_cast<unsigned int*>(take(16));
@@ -158,7 +164,7 @@ __device__ __forceinline__ void load_px(const uint16_t* p, int nv, float (&o)[PX
 // FULL: both stacks hold exactly NMAX frames (the usual case), so every "k < n" test below is a compile-time
 // constant: no predicates, no absent-entry selects (a quarter of the instructions of this issue-bound kernel)
 template <int NMAX, int MODE, int PX, bool FULL>
-__global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__ bias, int nb,
+__global__ void __launch_bounds__(masters_threads<NMAX>()) k_masters_bd(const uint16_t* __restrict__ bias, int nb,
                                                     const uint16_t* __restrict__ dark, int nd, int nf, Geom g,
                                                     MastersWs m, double r, float ksigma, int max_iter,
                                                     float* __restrict__ MB, float* __restrict__ MD)
@@ -221,7 +227,8 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
     // block partials of both planes; after the one barrier only warp 0 stays: it writes the partials and takes the ticket,
     // and in the LAST block to arrive it adds up all partials (fixed order) and turns them into 1/<G_k>.  (With the whole
     // block waiting for the fence + ticket round trip, "barrier" was the top stall reason of this kernel.)
-    __shared__ float2 s_w2[8];
+    constexpr int MT = masters_threads<NMAX>();
+    __shared__ float2 s_w2[MT / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     tb = warp_sum(tb);          // <= 64 values of one plane in float32: 1e-6 relative on a partial
     td = warp_sum(td);
@@ -231,7 +238,7 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
     int last = 0;
     if (lane == 0) {
         double sb = 0.0, sd = 0.0;
-        for (int i = 0; i < 8; ++i) { sb += (double)s_w2[i].x; sd += (double)s_w2[i].y; }
+        for (int i = 0; i < MT / 32; ++i) { sb += (double)s_w2[i].x; sd += (double)s_w2[i].y; }
         m.part_bd[2 * (size_t)blockIdx.x] = sb;
         m.part_bd[2 * (size_t)blockIdx.x + 1] = sd;
         __threadfence();
@@ -256,7 +263,7 @@ __global__ void __launch_bounds__(256) k_masters_bd(const uint16_t* __restrict__
 
 // ---- flat; the last block turns the block sums into 1/<MF_raw> ---------------------------------
 template <int NMAX, int MODE, int PX, bool FULL>
-__global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ flat, int nb, int nd, int nf, Geom g,
+__global__ void __launch_bounds__(masters_threads<NMAX>()) k_masters_f(const uint16_t* __restrict__ flat, int nb, int nd, int nf, Geom g,
                                                    MastersWs m, float r, float ksigma, int max_iter,
                                                    const float* __restrict__ MB, const float* __restrict__ MD,
                                                    float* __restrict__ MF)
@@ -303,7 +310,8 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
     float t = 0.f;
 #pragma unroll
     for (int i = 0; i < PX; ++i) t += mf[i];
-    __shared__ float s_w1[8];
+    constexpr int MT = masters_threads<NMAX>();
+    __shared__ float s_w1[MT / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     t = warp_sum(t);
     if (lane == 0) s_w1[warp] = t;
@@ -312,7 +320,7 @@ __global__ void __launch_bounds__(256) k_masters_f(const uint16_t* __restrict__ 
     int last = 0;
     if (lane == 0) {
         double sblk = 0.0;
-        for (int i = 0; i < 8; ++i) sblk += (double)s_w1[i];
+        for (int i = 0; i < MT / 32; ++i) sblk += (double)s_w1[i];
         m.part_f[blockIdx.x] = sblk;
         __threadfence();
         last = atomicAdd(m.ticket + 1, 1u) == gridDim.x - 1;
@@ -346,11 +354,11 @@ static void launch_bd(int mode, dim3 grid, cudaStream_t st, const uint16_t* bias
                       int nf, const Geom& g, const MastersWs& m, double r, float ks, int mi, float* MB, float* MD)
 {
     if (mode == MRED_MEDIAN)
-        k_masters_bd<NMAX, MRED_MEDIAN, PX, FULL><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
+        k_masters_bd<NMAX, MRED_MEDIAN, PX, FULL><<<grid, masters_threads<NMAX>(), 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
     else if (mode == MRED_MEAN)
-        k_masters_bd<NMAX, MRED_MEAN, PX, FULL><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
+        k_masters_bd<NMAX, MRED_MEAN, PX, FULL><<<grid, masters_threads<NMAX>(), 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
     else
-        k_masters_bd<NMAX, MRED_SIGCLIP, PX, FULL><<<grid, 256, 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
+        k_masters_bd<NMAX, MRED_SIGCLIP, PX, FULL><<<grid, masters_threads<NMAX>(), 0, st>>>(bias, nb, dark, nd, nf, g, m, r, ks, mi, MB, MD);
 }
 
 template <int NMAX, int PX, bool FULL>
@@ -358,11 +366,11 @@ static void launch_f(int mode, dim3 grid, cudaStream_t st, const uint16_t* flat,
                      const MastersWs& m, float r, float ks, int mi, const float* MB, const float* MD, float* MF)
 {
     if (mode == MRED_MEDIAN)
-        k_masters_f<NMAX, MRED_MEDIAN, PX, FULL><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
+        k_masters_f<NMAX, MRED_MEDIAN, PX, FULL><<<grid, masters_threads<NMAX>(), 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
     else if (mode == MRED_MEAN)
-        k_masters_f<NMAX, MRED_MEAN, PX, FULL><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
+        k_masters_f<NMAX, MRED_MEAN, PX, FULL><<<grid, masters_threads<NMAX>(), 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
     else
-        k_masters_f<NMAX, MRED_SIGCLIP, PX, FULL><<<grid, 256, 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
+        k_masters_f<NMAX, MRED_SIGCLIP, PX, FULL><<<grid, masters_threads<NMAX>(), 0, st>>>(flat, nb, nd, nf, g, m, r, ks, mi, MB, MD, MF);
 }
 
 // capacity buckets (the sorting network and every sweep are unrolled over the capacity, so a tight bucket
@@ -403,18 +411,18 @@ int launch_build_masters(const Geom& g, const uint16_t* bias, int nb, const uint
     const double rd = (double)t_flat / (double)t_dark;
 #define CALL_BD(N, PX)                                                                                         \
     do {                                                                                                       \
-        if (PX == 2 && pair_ok && nb == N && nd == N) launch_bd<N, PX, PX == 2>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
-        else if (PX == 2 && pair_ok) launch_bd<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
-        else launch_bd<N, 1, false>(o.mode, dim3((unsigned)((np + 255) / 256)), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        if (PX == 2 && pair_ok && nb == N && nd == N) launch_bd<N, PX, PX == 2>(o.mode, dim3((unsigned)((np / 2 + masters_threads<N>() - 1) / masters_threads<N>())), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        else if (PX == 2 && pair_ok) launch_bd<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + masters_threads<N>() - 1) / masters_threads<N>())), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
+        else launch_bd<N, 1, false>(o.mode, dim3((unsigned)((np + masters_threads<N>() - 1) / masters_threads<N>())), st, bias, nb, dark, nd, nf, g, m, rd, o.ksigma, o.max_iter, MB, MD); \
     } while (0)
     MRED_BUCKET(nbd, CALL_BD);
 #undef CALL_BD
     MRED_LAUNCH_CHECK();
 #define CALL_F(N, PX)                                                                                          \
     do {                                                                                                       \
-        if (PX == 2 && pair_ok && nf == N) launch_f<N, PX, PX == 2>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
-        else if (PX == 2 && pair_ok) launch_f<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
-        else launch_f<N, 1, false>(o.mode, dim3((unsigned)((np + 255) / 256)), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        if (PX == 2 && pair_ok && nf == N) launch_f<N, PX, PX == 2>(o.mode, dim3((unsigned)((np / 2 + masters_threads<N>() - 1) / masters_threads<N>())), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        else if (PX == 2 && pair_ok) launch_f<N, PX, false>(o.mode, dim3((unsigned)((np / 2 + masters_threads<N>() - 1) / masters_threads<N>())), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
+        else launch_f<N, 1, false>(o.mode, dim3((unsigned)((np + masters_threads<N>() - 1) / masters_threads<N>())), st, flat, nb, nd, nf, g, m, r, o.ksigma, o.max_iter, MB, MD, MF); \
     } while (0)
     MRED_BUCKET(nf, CALL_F);
 #undef CALL_F
