@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--no-graph", action="store_true", help="plain launches in the timed region instead of a CUDA graph replay")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the short runs of configs 2 and 5 reported under `extra`")
+    ap.add_argument("--no-extra", action="store_true", help="skip the short runs of the other configs (1, 2, 4, 5) and of the bad-pixel fill reported under `extra`")
     return ap.parse_args()
 
 
@@ -546,7 +546,7 @@ def run_ours(args):
     # the other single-GPU configs, shorter runs of the same step, so that the driver's line carries them too
     extra = {}
     if rank == 0 and world == 1 and not args.no_extra:
-        for c in (2, 5):
+        for c in (1, 2, 4, 5):
             if c == cfg:
                 continue
             try:
