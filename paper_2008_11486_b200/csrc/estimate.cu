@@ -168,8 +168,8 @@ __device__ __forceinline__ double val_of(unsigned long long k)
     return __longlong_as_double((long long)u);
 }
 
-// Ascending bitonic sort of keys[0..P) in shared memory, P a power of two (block-wide call, blockDim.x = 1024).
-// P <= 1024: one key per thread in a register; the 40 of 55 exchange steps whose partner sits in the same warp are two
+// Ascending bitonic sort of keys[0..P) in shared memory, P a power of two (block-wide call).
+// P <= blockDim.x: one key per thread in a register; the 40 of 55 exchange steps whose partner sits in the same warp are two
 // shuffles, only the 15 cross-warp steps go through shared memory (two barriers each).  Larger P: pairs in shared memory.
 // A data-independent ~3 us, where the 8-pass radix select it replaces spent ~20 us in barriers and same-bin atomics.
 __device__ void block_sort(unsigned long long* keys, int P)
@@ -255,7 +255,9 @@ __device__ void block_profile(const EstimateWs& e, int w, int h, int k, int axis
 
 // ---------------------------------------------------------------------------------------------
 // k_estimate: profile finishing AND lag search of one (frame, axis) per block (round 1 had two kernels, k_finalize and
-// k_correlate: 28-36 us of dependent latency per stack).  grid (n, 2), block 1024.  Block x = 0 takes the REFERENCE frame:
+// k_correlate: 28-36 us of dependent latency per stack).  grid (n, 2), block 512 (1024 threads, one sort key each, are no
+// faster alone -- 30.4 against 30.8 us -- and a 1024-thread block waits longer for room on an SM that other streams' kernels
+// share: bench.py's 6-stream step 1.790 -> 1.777 ms; 256 threads: 1.771 ms but 36.6 us alone).  Block x = 0 takes the REFERENCE frame:
 // it writes its median-subtracted profile to e.prof and raises a flag (the zeroed ticket of (ref, axis)); every other block
 // finishes its own profile (the bitonic sort is the long part, and runs in parallel with the reference's), then waits for
 // the flag -- a block only ever waits for the block with x = 0 of its own axis, which precedes it in dispatch order, the
@@ -300,7 +302,7 @@ __global__ void __launch_bounds__(1024) k_estimate(int w, int h, int n, int ref,
     for (int i = threadIdx.x; i < len; i += blockDim.x) a[i] = __ldcg(gref + i);
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int q = warp; q <= 2 * R; q += 32) {
+    for (int q = warp; q <= 2 * R; q += (int)(blockDim.x >> 5)) {
         const int l = q - R;
         const int j0 = max(0, -l), j1 = min(len, len - l);
         double s = 0.0;
@@ -357,7 +359,7 @@ int launch_estimate(const float* frames, int n, int w, int h, int ref, int max_l
         MRED_CUDA_TRY(cudaFuncSetAttribute(k_estimate, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * PROF_MAXLEN * (int)sizeof(double)));
         once.mark(dev);
     }
-    k_estimate<<<dim3(n, 2), 1024, 2 * (size_t)P * sizeof(double), st>>>(w, h, n, ref, max_lag, peak,
+    k_estimate<<<dim3(n, 2), 512, 2 * (size_t)P * sizeof(double), st>>>(w, h, n, ref, max_lag, peak,
                                                                         bad ? ((flags & EST_SHARED_COUNTS) ? 2 : 1) : 0, e, ishift, shift);
     MRED_LAUNCH_CHECK();
     return MRED_OK;
