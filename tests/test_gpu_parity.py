@@ -162,6 +162,19 @@ def test_build_masters_parity(gname, nm, mode):
     assert abs(float(host(MF).astype(np.float64).mean()) - 1.0) < 1e-6
 
 
+@pytest.mark.parametrize("mode", [0, 2])
+@pytest.mark.parametrize("gname,nm", [("small", 33), ("ragged", 48), ("small", 64), ("ragged", 100), ("small", 130), ("small", 255)])
+def test_build_masters_long_columns(gname, nm, mode):
+    # the one-pixel-per-thread capacity buckets (48, 64, 128, 256) of the combine kernels, full and partly filled
+    g = GEOMS[gname]
+    grp = synth.make_group(2, 1, geom=g, n_master=nm, science=False)
+    ref = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat, mode=mode)
+    MB, MD, MF = mred.build_masters(g, dev(grp.bias), dev(grp.dark), grp.t_dark, dev(grp.flat), grp.t_flat, mode=mode)
+    assert_close(host(MB), ref.MB, "MB")
+    assert_close(host(MD), ref.MD, "MD")
+    assert_close(host(MF), ref.MF, "MF")
+
+
 def test_build_masters_unequal_counts_and_identical_frames():
     g = GEOMS["small"]
     grp = synth.make_group(1, geom=g, n_master=9, science=False)
