@@ -78,6 +78,29 @@ __device__ __forceinline__ Combined combine_median(float (&v)[NMAX], int m)
     return r;
 }
 
+// Median of a partly filled column whose absent slots the caller has PADDED ON BOTH SIDES: of the NMAX - n absent slots,
+// L = (NMAX - n) >> 1 hold -INF and the others +INF (pad_slot below).  The n values then sort into slots [L, L + n), and the
+// middle of that range is the same pair of slots whatever n is -- so, as for a full column, the outputs are compile-time
+// slots and the compiler prunes the network to the comparators that reach them (the +INF-only padding of combine_median
+// moves the middle with n: every slot is a possible output, the whole network stays).  n >= 1.
+//   NMAX even: slots NMAX/2 - 1 and NMAX/2 for even n, slot NMAX/2 - 1 alone for odd n;
+//   NMAX odd:  slot (NMAX-1)/2 alone for odd n, slots (NMAX-3)/2 and (NMAX-1)/2 for even n.
+template <int NMAX>
+__device__ __forceinline__ float pad_slot(int k, int n)      // value of absent slot k >= n
+{
+    return k < n + ((NMAX - n) >> 1) ? -CUDART_INF_F : CUDART_INF_F;
+}
+template <int NMAX>
+__device__ __forceinline__ float median_padded(float (&v)[NMAX], int n)
+{
+    sort_network<NMAX>(v);
+    float a, b;
+    if (NMAX == 1) { a = v[0]; b = a; }
+    else if (NMAX % 2 == 0) { a = v[NMAX / 2 - 1]; b = (n & 1) ? a : v[NMAX / 2]; }
+    else { b = v[(NMAX - 1) / 2]; a = (n & 1) ? b : v[NMAX >= 3 ? (NMAX - 3) / 2 : 0]; }
+    return 0.5f * a + 0.5f * b;                      // a == b for odd n: exact
+}
+
 // Median-centred clip (Q29): each pass is centred on the median of the survivors, sigma =
 // their r.m.s. about it, keep |v - med| <= k sigma; the result is the mean of the survivors.  The column is SORTED once
 // (absent entries hold +INF and sort to the end); a pass can only reject from the two ends of the sorted survivors, so
