@@ -197,11 +197,13 @@ __global__ void __launch_bounds__(masters_threads<NMAX>()) k_masters_bd(const ui
         const int nv = min(PX, g.w - x);
         const size_t q = (size_t)(y + g.y0) * g.W + (x + g.x0);
         const size_t p = (size_t)y * g.w + x;
-        float v[PX][NMAX], dk[PX][NMAX];
+        // up to 32 frames every load of both stacks is issued before the first median starts (address = base + k * frame:
+        // one multiply-add per load); longer columns load the darks after the bias median -- two columns of 64+ values do
+        // not fit the register file together (128 frames: 255 registers and spills with both, 167 without: 1.45 -> 1.00 ms)
+        constexpr bool BOTH = NMAX <= 32;
+        float v[PX][NMAX], dk[PX][BOTH ? NMAX : 1];
         const uint16_t* pb = bias + q;
         const uint16_t* pd = dark + q;
-        // every load of both stacks is issued before the first median starts (address = base + k * frame: one
-        // multiply-add per load)
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
             float o[PX], od[PX];
@@ -211,16 +213,23 @@ __global__ void __launch_bounds__(masters_threads<NMAX>()) k_masters_bd(const ui
             // the load: ptxas put the conversion of a predicated load right behind it, so a thread had ONE load in
             // flight at a time (64 frames: 945 us for this kernel, 3 % of the DRAM bandwidth, every warp waiting)
             load_px<PX>(frame_ptr(pb, FULL ? k : min(k, nb - 1), fsb), nv, o);
-            load_px<PX>(frame_ptr(pd, FULL ? k : min(k, nd - 1), fsb), nv, od);
+            if (BOTH) load_px<PX>(frame_ptr(pd, FULL ? k : min(k, nd - 1), fsb), nv, od);
 #pragma unroll
-            for (int i = 0; i < PX; ++i) { v[i][k] = (FULL || k < nb) ? o[i] - s_lb[k] : absent_slot<NMAX, MODE>(k, nb); dk[i][k] = od[i]; }
+            for (int i = 0; i < PX; ++i) {
+                v[i][k] = (FULL || k < nb) ? o[i] - s_lb[k] : absent_slot<NMAX, MODE>(k, nb);
+                if (BOTH) dk[i][k] = od[i];
+            }
         }
 #pragma unroll
         for (int i = 0; i < PX; ++i) mb[i] = combine_all<NMAX, MODE>(v[i], FULL ? NMAX : nb, ksigma, max_iter);
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
+            float od[PX];
 #pragma unroll
-            for (int i = 0; i < PX; ++i) v[i][k] = (FULL || k < nd) ? (dk[i][k] - s_ld[k]) - mb[i] : absent_slot<NMAX, MODE>(k, nd);
+            for (int i = 0; i < PX; ++i) od[i] = BOTH ? dk[i][k] : 0.f;
+            if (!BOTH) load_px<PX>(frame_ptr(pd, FULL ? k : min(k, nd - 1), fsb), nv, od);
+#pragma unroll
+            for (int i = 0; i < PX; ++i) v[i][k] = (FULL || k < nd) ? (od[i] - s_ld[k]) - mb[i] : absent_slot<NMAX, MODE>(k, nd);
         }
 #pragma unroll
         for (int i = 0; i < PX; ++i) md[i] = combine_all<NMAX, MODE>(v[i], FULL ? NMAX : nd, ksigma, max_iter);
@@ -402,7 +411,9 @@ static void launch_f(int mode, dim3 grid, cudaStream_t st, const uint16_t* flat,
         else if ((n) <= 32) { CALL(32, 2); }     \
         else if ((n) <= 48) { CALL(48, 1); }     \
         else if ((n) <= 64) { CALL(64, 1); }     \
+        else if ((n) <= 96) { CALL(96, 1); }     \
         else if ((n) <= 128) { CALL(128, 1); }   \
+        else if ((n) <= 192) { CALL(192, 1); }   \
         else { CALL(256, 1); }                   \
     } while (0)
 

@@ -163,9 +163,9 @@ def test_build_masters_parity(gname, nm, mode):
 
 
 @pytest.mark.parametrize("mode", [0, 2])
-@pytest.mark.parametrize("gname,nm", [("small", 33), ("ragged", 48), ("small", 64), ("ragged", 100), ("small", 130), ("small", 255)])
+@pytest.mark.parametrize("gname,nm", [("small", 33), ("ragged", 48), ("small", 64), ("ragged", 80), ("small", 96), ("ragged", 100), ("small", 130), ("ragged", 192), ("small", 255)])
 def test_build_masters_long_columns(gname, nm, mode):
-    # the one-pixel-per-thread capacity buckets (48, 64, 128, 256) of the combine kernels, full and partly filled
+    # the one-pixel-per-thread capacity buckets (48, 64, 96, 128, 192, 256) of the combine kernels, full and partly filled
     g = GEOMS[gname]
     grp = synth.make_group(2, 1, geom=g, n_master=nm, science=False)
     ref = oracle.build_masters(g, grp.bias, grp.dark, grp.t_dark, grp.flat, grp.t_flat, mode=mode)
