@@ -66,9 +66,9 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
             if (x >= f.x && x <= f.y && y >= f.z && y <= f.w) inside[i] |= 1u << b;
         }
     }
-    int m = 0;
+    int m = 0, nin = 0;                                    // nin: frames that cover every pixel of the block (block-uniform)
 #pragma unroll
-    for (int i = 0; i < NW; ++i) m += __popc(inside[i]);
+    for (int i = 0; i < NW; ++i) { m += __popc(inside[i]); nin += __popc(s_in[i]); }
     const float* src = stack + p;
     if (MODE != MRED_MEDIAN && MODE != MRED_MEDCLIP && NMAX <= 24 && n == NMAX && m == NMAX) {
         // short column, every frame covers this pixel (the usual case; with 32+ frames some lane of the warp
@@ -86,6 +86,24 @@ __global__ void __launch_bounds__(256) k_coadd(const float* __restrict__ stack, 
             }
             return;
         }
+    } else if (MODE == MRED_MEDIAN && NMAX <= 64 && nin == n) {
+        // median, every frame covers the whole block (block-uniform, the usual case): the absent slots are exactly k >= n,
+        // so they can be padded on both sides (combine.cuh, median_padded) and the network is pruned to the two middle
+        // slots at compile time.  Bit-identical to the general path: the median is the same value either way.
+#pragma unroll
+        for (int k = 0; k < NMAX; ++k) {
+            v[k] = k < n ? __ldcs(src) : pad_slot<NMAX>(k, n);
+            src += np;
+        }
+        out[p] = median_padded<NMAX>(v, n);
+        if (count) count[p] = (uint16_t)n;
+        if (rejmask) {
+            const int words = (n + 31) >> 5;
+#pragma unroll
+            for (int i = 0; i < NW; ++i)
+                if (i < words) rejmask[(size_t)i * np + p] = 0u;
+        }
+        return;
     } else {
 #pragma unroll
         for (int k = 0; k < NMAX; ++k) {
