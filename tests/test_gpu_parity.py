@@ -175,6 +175,24 @@ def test_build_masters_long_columns(gname, nm, mode):
     assert_close(host(MF), ref.MF, "MF")
 
 
+@pytest.mark.parametrize("counts", [(1, 1, 1), (1, 2, 3), (2, 3, 1), (2, 2, 2), (4, 5, 2), (5, 4, 4), (6, 3, 5), (7, 8, 6),
+                                    (9, 12, 11), (13, 16, 15), (17, 19, 20), (21, 24, 23), (25, 31, 32), (33, 40, 47),
+                                    (49, 63, 64)])
+def test_build_masters_partly_filled_buckets(counts):
+    # every parity of (bucket capacity, frame count): the median of a partly filled bucket reads fixed middle slots of a
+    # column padded with -INF / +INF (combine.cuh, median_padded), odd and even capacities alike
+    g = GEOMS["small"]
+    nb, nd, nf = counts
+    grp = synth.make_group(2, 2, geom=g, n_master=max(counts), science=False)
+    b, d, f = grp.bias[:nb], grp.dark[:nd], grp.flat[:nf]
+    for mode in (0, 2):
+        ref = oracle.build_masters(g, b, d, grp.t_dark, f, grp.t_flat, mode=mode)
+        MB, MD, MF = mred.build_masters(g, dev(b), dev(d), grp.t_dark, dev(f), grp.t_flat, mode=mode)
+        assert_close(host(MB), ref.MB, "MB %s mode %d" % (counts, mode))
+        assert_close(host(MD), ref.MD, "MD %s mode %d" % (counts, mode))
+        assert_close(host(MF), ref.MF, "MF %s mode %d" % (counts, mode))
+
+
 def test_build_masters_unequal_counts_and_identical_frames():
     g = GEOMS["small"]
     grp = synth.make_group(1, geom=g, n_master=9, science=False)
